@@ -1,0 +1,235 @@
+"""fp64 CPU oracle for the cone-beam operators -- TEST INFRASTRUCTURE ONLY.
+
+Thin ctypes wrapper around ``oracle/cbct_oracle.c`` (plain C, fp64, OpenMP).
+Only ``tests/``, ``__graft_entry__.smoke()`` and ``bench.py``'s
+``cpu_baseline`` / ``--impl reference`` legs may import this package.  It
+imports nothing from ``paper_2512_21180_b200`` and shares no code with the
+CUDA path.  Definitions: PAPER.md:85-89 (Eq. 5), PAPER.md:61 (geometry),
+PAPER.md:157/181/397 (FDK); discretisation readings R1-R11 in DESIGN.md s.3.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+from dataclasses import dataclass, field
+from typing import Optional, Sequence
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "cbct_oracle.c")
+_LIB = os.path.join(_HERE, "libcbct_oracle.so")
+
+
+def build(force: bool = False) -> str:
+    """Compile the oracle with gcc (-O2 -fopenmp).  Returns the .so path."""
+    if (not force and os.path.exists(_LIB)
+            and os.path.getmtime(_LIB) >= os.path.getmtime(_SRC)):
+        return _LIB
+    tmp = _LIB + ".tmp%d" % os.getpid()
+    cmd = ["gcc", "-O2", "-std=c99", "-fopenmp", "-fPIC", "-shared", "-D_GNU_SOURCE",
+           "-o", tmp, _SRC, "-lm"]
+    subprocess.run(cmd, check=True)
+    os.replace(tmp, _LIB)
+    return _LIB
+
+
+class _CGeom(ctypes.Structure):
+    _fields_ = [
+        ("sid_mm", ctypes.c_double), ("sdd_mm", ctypes.c_double),
+        ("n_views", ctypes.c_int32),
+        ("angles_rad", ctypes.POINTER(ctypes.c_double)),
+        ("det_nu", ctypes.c_int32), ("det_nv", ctypes.c_int32),
+        ("det_du_mm", ctypes.c_double), ("det_dv_mm", ctypes.c_double),
+        ("det_off_u_mm", ctypes.c_double), ("det_off_v_mm", ctypes.c_double),
+        ("vol_nx", ctypes.c_int32), ("vol_ny", ctypes.c_int32), ("vol_nz", ctypes.c_int32),
+        ("vox_mm", ctypes.c_double),
+        ("vol_cx_mm", ctypes.c_double), ("vol_cy_mm", ctypes.c_double), ("vol_cz_mm", ctypes.c_double),
+        ("step_vox", ctypes.c_double),
+    ]
+
+
+@dataclass
+class Geom:
+    """Geometry descriptor of the oracle (its own type; mirrors PAPER.md:61)."""
+    sid_mm: float = 1000.0
+    sdd_mm: float = 1536.0
+    n_views: int = 36
+    det_nu: int = 48
+    det_nv: int = 48
+    det_du_mm: float = 3.2
+    det_dv_mm: float = 3.2
+    det_off_u_mm: float = 0.0
+    det_off_v_mm: float = 0.0
+    vol_nx: int = 32
+    vol_ny: int = 32
+    vol_nz: int = 32
+    vox_mm: float = 4.0
+    vol_cx_mm: float = 0.0
+    vol_cy_mm: float = 0.0
+    vol_cz_mm: float = 0.0
+    step_vox: float = 0.5
+    angles_rad: Optional[Sequence[float]] = None
+    _keep: list = field(default_factory=list, repr=False, compare=False)
+
+    def vol_shape(self, channels: int = 1):
+        return (channels, self.vol_nz, self.vol_ny, self.vol_nx)
+
+    def sino_shape(self, channels: int = 1):
+        return (channels, self.n_views, self.det_nv, self.det_nu)
+
+    def _c(self) -> _CGeom:
+        c = _CGeom()
+        for name, _ in _CGeom._fields_:
+            if name == "angles_rad":
+                continue
+            setattr(c, name, getattr(self, name))
+        if self.angles_rad is not None:
+            a = np.ascontiguousarray(np.asarray(self.angles_rad, dtype=np.float64))
+            assert a.shape == (self.n_views,)
+            self._keep.append(a)
+            c.angles_rad = a.ctypes.data_as(ctypes.POINTER(ctypes.c_double))
+        else:
+            c.angles_rad = ctypes.POINTER(ctypes.c_double)()
+        return c
+
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        L = ctypes.CDLL(build())
+        dp = ctypes.POINTER(ctypes.c_double)
+        ip = ctypes.POINTER(ctypes.c_int64)
+        gp = ctypes.POINTER(_CGeom)
+        L.oracle_max_threads.restype = ctypes.c_int
+        L.oracle_fp.argtypes = [gp, dp, dp, ctypes.c_int, ctypes.c_int]
+        L.oracle_fp_rays.argtypes = [gp, dp, ctypes.c_int, ip, ctypes.c_int64, dp]
+        L.oracle_count_samples.argtypes = [gp, ctypes.c_int]
+        L.oracle_count_samples.restype = ctypes.c_int64
+        L.oracle_bp_adjoint.argtypes = [gp, dp, dp, ctypes.c_int, ctypes.c_int]
+        L.oracle_bp_adjoint_voxels.argtypes = [gp, dp, ctypes.c_int, ip, ctypes.c_int64, dp]
+        L.oracle_bp_fdk.argtypes = [gp, dp, dp, ctypes.c_int]
+        L.oracle_bp_fdk_voxels.argtypes = [gp, dp, ctypes.c_int, ip, ctypes.c_int64, dp]
+        _lib = L
+    return _lib
+
+
+def _dptr(a):
+    return a.ctypes.data_as(ctypes.POINTER(ctypes.c_double))
+
+
+def _iptr(a):
+    return a.ctypes.data_as(ctypes.POINTER(ctypes.c_int64))
+
+
+def _as_f64(a, shape_tail):
+    a = np.ascontiguousarray(np.asarray(a, dtype=np.float64))
+    if a.ndim == len(shape_tail):
+        a = a[None]
+    assert a.shape[1:] == tuple(shape_tail), (a.shape, shape_tail)
+    return a
+
+
+def max_threads() -> int:
+    return int(lib().oracle_max_threads())
+
+
+def fp(g: Geom, vol, clip: bool = True) -> np.ndarray:
+    """A2: vol[C,nz,ny,nx] -> sino[C,n_views,nv,nu] (fp64)."""
+    vol = _as_f64(vol, g.vol_shape()[1:])
+    out = np.empty(g.sino_shape(vol.shape[0]), dtype=np.float64)
+    cg = g._c()
+    rc = lib().oracle_fp(ctypes.byref(cg), _dptr(vol), _dptr(out), vol.shape[0], int(clip))
+    assert rc == 0
+    return out
+
+
+def fp_rays(g: Geom, vol, ray_idx) -> np.ndarray:
+    """A2 at selected flat ray indices ((i*nv+iv)*nu+iu) -> out[C, n_rays]."""
+    vol = _as_f64(vol, g.vol_shape()[1:])
+    idx = np.ascontiguousarray(np.asarray(ray_idx, dtype=np.int64))
+    out = np.empty((vol.shape[0], idx.size), dtype=np.float64)
+    cg = g._c()
+    rc = lib().oracle_fp_rays(ctypes.byref(cg), _dptr(vol), vol.shape[0], _iptr(idx), idx.size, _dptr(out))
+    assert rc == 0
+    return out
+
+
+def count_samples(g: Geom, clip: bool = True) -> int:
+    """Number of (ray, k) samples with -1 < q < N on every axis (one channel)."""
+    cg = g._c()
+    return int(lib().oracle_count_samples(ctypes.byref(cg), int(clip)))
+
+
+def bp_adjoint(g: Geom, sino, clip: bool = True) -> np.ndarray:
+    """A3: sino[C,n_views,nv,nu] -> vol[C,nz,ny,nx] (fp64), exact transpose of fp."""
+    sino = _as_f64(sino, g.sino_shape()[1:])
+    out = np.empty(g.vol_shape(sino.shape[0]), dtype=np.float64)
+    cg = g._c()
+    rc = lib().oracle_bp_adjoint(ctypes.byref(cg), _dptr(sino), _dptr(out), sino.shape[0], int(clip))
+    assert rc == 0
+    return out
+
+
+def bp_adjoint_voxels(g: Geom, sino, vox_idx) -> np.ndarray:
+    """A3 at selected flat voxel indices ((iz*ny+iy)*nx+ix) -> out[C, n_vox]."""
+    sino = _as_f64(sino, g.sino_shape()[1:])
+    idx = np.ascontiguousarray(np.asarray(vox_idx, dtype=np.int64))
+    out = np.empty((sino.shape[0], idx.size), dtype=np.float64)
+    cg = g._c()
+    rc = lib().oracle_bp_adjoint_voxels(ctypes.byref(cg), _dptr(sino), sino.shape[0], _iptr(idx),
+                                        idx.size, _dptr(out))
+    assert rc == 0
+    return out
+
+
+def bp_fdk(g: Geom, sino) -> np.ndarray:
+    """A4: FDK-weighted voxel-driven backprojection (backprojection stage only)."""
+    sino = _as_f64(sino, g.sino_shape()[1:])
+    out = np.empty(g.vol_shape(sino.shape[0]), dtype=np.float64)
+    cg = g._c()
+    rc = lib().oracle_bp_fdk(ctypes.byref(cg), _dptr(sino), _dptr(out), sino.shape[0])
+    assert rc == 0
+    return out
+
+
+def bp_fdk_voxels(g: Geom, sino, vox_idx) -> np.ndarray:
+    """A4 at selected flat voxel indices -> out[C, n_vox]."""
+    sino = _as_f64(sino, g.sino_shape()[1:])
+    idx = np.ascontiguousarray(np.asarray(vox_idx, dtype=np.int64))
+    out = np.empty((sino.shape[0], idx.size), dtype=np.float64)
+    cg = g._c()
+    rc = lib().oracle_bp_fdk_voxels(ctypes.byref(cg), _dptr(sino), sino.shape[0], _iptr(idx),
+                                    idx.size, _dptr(out))
+    assert rc == 0
+    return out
+
+
+def fdk_frontend(g: Geom, proj) -> np.ndarray:
+    """Caller-side FDK steps (reading R11; textbook Feldkamp, ref [9] PAPER.md:397;
+    ramp taps as in Kak & Slaney eq. 61 for equispaced flat detectors):
+      p~ = p * SDD / sqrt(SDD^2 + u^2 + v^2)         (cosine weight)
+      q  = a * (h * p~) along u,  a = du*SID/SDD,     (ramp filter, virtual
+           h[0] = 1/(4 a^2), h[odd n] = -1/(pi^2 n^2 a^2), h[even] = 0   detector at isocentre)
+    and the reconstruction is (dphi/2) * bp_fdk(q).  proj[n_views,nv,nu] fp64."""
+    proj = np.asarray(proj, dtype=np.float64)
+    nu, nv = g.det_nu, g.det_nv
+    u = (np.arange(nu) - 0.5 * (nu - 1)) * g.det_du_mm + g.det_off_u_mm
+    v = (np.arange(nv) - 0.5 * (nv - 1)) * g.det_dv_mm + g.det_off_v_mm
+    cosw = g.sdd_mm / np.sqrt(g.sdd_mm ** 2 + u[None, :] ** 2 + v[:, None] ** 2)
+    pt = proj * cosw[None]
+    a = g.det_du_mm * g.sid_mm / g.sdd_mm
+    n = np.arange(-(nu - 1), nu)
+    h = np.zeros(n.shape, dtype=np.float64)
+    h[n == 0] = 1.0 / (4.0 * a * a)
+    odd = (n % 2) != 0
+    h[odd] = -1.0 / (np.pi ** 2 * n[odd].astype(np.float64) ** 2 * a * a)
+    out = np.empty_like(pt)
+    for i in range(pt.shape[0]):
+        for r in range(nv):
+            out[i, r] = a * np.convolve(pt[i, r], h)[nu - 1:2 * nu - 1]
+    return out

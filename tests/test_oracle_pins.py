@@ -1,0 +1,286 @@
+"""Pins for the fp64 oracle (CPU only): closed forms, invariants, brute force.
+
+Each test would fail under a plausible mistake in oracle/cbct_oracle.c (a
+dropped term, wrong sign/index, transposed operand, half-voxel slip).  Pin
+numbers P1..P12 follow SURVEY.md s.8(c) / DESIGN.md s.5.
+"""
+import os
+
+import numpy as np
+import pytest
+
+from paper_2512_21180_b200 import synth
+from tests import analytic as an
+
+TINY = synth.geom_kwargs(synth.CONFIGS["tiny"])
+
+
+def G(oracle, **over):
+    kw = dict(TINY)
+    kw.update(over)
+    return oracle.Geom(**kw), kw
+
+
+def test_golden_paper_geometry():
+    """Configs carry the constants the paper prints."""
+    gold = {}
+    path = os.path.join(os.path.dirname(__file__), "golden", "paper_geometry.txt")
+    for line in open(path):
+        line = line.split("#")[0].split()
+        if len(line) == 2:
+            gold[line[0]] = float(line[1])
+    c = synth.CONFIGS["pyramid_256"]
+    assert c["sid_mm"] == gold["sid_mm"]
+    assert c["sdd_mm"] - c["sid_mm"] == gold["iso_det_mm"]
+    assert c["det_off_u_mm"] == gold["det_offset_mm"]
+    assert c["det_nu"] == c["det_nv"] == gold["panel_pixels"]
+    assert abs(c["det_nu"] * c["det_du_mm"] - gold["panel_side_mm"]) < 1e-9
+    assert c["vol_nx"] == gold["volume_voxels"] and c["vox_mm"] == gold["voxel_mm"]
+
+
+def test_p1_ball_central_chord(oracle_mod):
+    """P1: central ray through a centred ball = chord * density = 2 r rho."""
+    o = oracle_mod
+    g, kw = G(o, det_nu=49, det_nv=49, n_views=4)
+    ball = [(np.zeros(3), np.full(3, 40.0), np.eye(3), 0.02)]
+    vol = synth.rasterise(ball, 32, 4.0).astype(np.float64)
+    s = o.fp(g, vol)[0]
+    for i in range(4):
+        assert abs(s[i, 24, 24] - 1.6) / 1.6 < 2e-3
+    # a ray that misses the grid entirely integrates to exactly zero
+    gw, _ = G(o, det_nu=49, det_nv=49, n_views=1, det_off_u_mm=600.0)
+    assert o.fp(gw, vol)[0, 0, 24, 48] == 0.0
+
+
+def test_p2_ellipsoid_sinogram_converges(oracle_mod):
+    """P2: rasterised ellipsoids -> analytic chord sinogram as h -> 0 (O(h))."""
+    o = oracle_mod
+    ell = synth.draw_ellipsoids(7, 4, 100.0, 3.0)
+    errs = []
+    for n, h in ((32, 4.0), (64, 2.0), (128, 1.0)):
+        g, kw = G(o, vol_nx=n, vol_ny=n, vol_nz=n, vox_mm=h, n_views=6)
+        vol = synth.rasterise(ell, n, h).astype(np.float64)
+        errs.append(an.rel_l2(o.fp(g, vol)[0], an.ellipsoid_sinogram(kw, ell)))
+    assert errs[0] < 0.10 and errs[2] < 0.025, errs
+    assert errs[0] > 1.4 * errs[1] > 1.4 * 1.4 * errs[2] * 0.7, errs
+
+
+def test_p3_gaussian_blob(oracle_mod):
+    """P3: smooth blob, O(h^2) convergence; a half-voxel slip is unmistakable."""
+    o = oracle_mod
+    centre, sigma, rho = (30.0, -20.0, 10.0), 16.0, 0.02
+    errs = {}
+    for n, h in ((64, 4.0), (128, 2.0)):
+        g, kw = G(o, vol_nx=n, vol_ny=n, vol_nz=n, vox_mm=h, n_views=5,
+                  det_nu=64, det_nv=64, det_du_mm=4.0, det_dv_mm=4.0, det_off_u_mm=12.0)
+        vol = an.gaussian_volume(n, h, centre, sigma, rho)
+        errs[n] = an.rel_l2(o.fp(g, vol)[0], an.gaussian_sinogram(kw, centre, sigma, rho))
+    assert errs[64] < 1.2e-2, errs
+    assert errs[128] < errs[64] / 3.5, errs
+    # mutation: the volume sampled on a grid slipped by half a voxel
+    g, kw = G(o, vol_nx=64, vol_ny=64, vol_nz=64, vox_mm=4.0, n_views=5,
+              det_nu=64, det_nv=64, det_du_mm=4.0, det_dv_mm=4.0, det_off_u_mm=12.0)
+    bad = an.gaussian_volume(64, 4.0, centre, sigma, rho, shift_vox=0.5)
+    e_bad = an.rel_l2(o.fp(g, bad)[0], an.gaussian_sinogram(kw, centre, sigma, rho))
+    assert e_bad > 4.0 * errs[64], (e_bad, errs)
+
+
+def test_p3b_orientation_of_axes(oracle_mod):
+    """A blob off-centre on one axis at a time lands where the geometry says:
+    pins the sign of e_u, the u/v order of the sinogram and the z axis."""
+    o = oracle_mod
+    g, kw = G(o, n_views=4, det_nu=48, det_nv=48)
+    for centre in ((24.0, 5.0, -7.0), (-6.0, 24.0, 5.0), (5.0, -7.0, 24.0)):
+        vol = an.gaussian_volume(32, 4.0, centre, 8.0, 0.02)
+        s = o.fp(g, vol)[0]
+        ref = an.gaussian_sinogram(kw, centre, 8.0, 0.02)
+        for i in range(4):
+            assert np.unravel_index(np.argmax(s[i]), s[i].shape) == \
+                np.unravel_index(np.argmax(ref[i]), ref[i].shape)
+        assert an.rel_l2(s, ref) < 0.05
+
+
+def test_p4_adjoint_identity(oracle_mod):
+    """P4: <A x, y> = <x, A^T y> to 1e-12 (half-fan offset, off-centre volume)."""
+    o = oracle_mod
+    g, _ = G(o, det_off_u_mm=31.0, det_off_v_mm=-5.0, vol_cx_mm=3.0, vol_cy_mm=-7.0,
+             vol_cz_mm=2.0, n_views=7, vol_nx=20, vol_ny=24, vol_nz=16, det_nu=40, det_nv=36)
+    rng = np.random.default_rng(5)
+    x = rng.normal(size=g.vol_shape(2))
+    y = rng.normal(size=g.sino_shape(2))
+    lhs = float(np.sum(o.fp(g, x) * y))
+    rhs = float(np.sum(x * o.bp_adjoint(g, y)))
+    assert abs(lhs - rhs) / abs(lhs) < 1e-12
+
+
+def test_p5_explicit_matrix_transpose(oracle_mod):
+    """P5: build A column by column on 8^3 and compare A^T y entry by entry."""
+    o = oracle_mod
+    g, _ = G(o, vol_nx=8, vol_ny=8, vol_nz=8, det_nu=12, det_nv=10, det_du_mm=6.0,
+             det_dv_mm=6.5, n_views=5, det_off_u_mm=7.0, vol_cx_mm=1.0)
+    eye = np.eye(512).reshape(512, 8, 8, 8)
+    A = o.fp(g, eye).reshape(512, -1).T          # [n_rays, 512]
+    assert np.count_nonzero(A) > 0
+    rng = np.random.default_rng(11)
+    y = rng.random(g.sino_shape(1))
+    bt = o.bp_adjoint(g, y).reshape(-1)
+    ref = A.T @ y.reshape(-1)
+    assert np.max(np.abs(bt - ref)) <= 1e-12 * np.max(np.abs(ref))
+    # and the forward of a random volume is A x
+    x = rng.normal(size=(8, 8, 8))
+    assert np.max(np.abs(o.fp(g, x).reshape(-1) - A @ x.reshape(-1))) < 1e-12
+
+
+def test_p6_fourfold_view_symmetry(oracle_mod):
+    """P6: a grid with 4-fold symmetry about z gives identical views 90 deg apart."""
+    o = oracle_mod
+    ball = [(np.zeros(3), np.full(3, 40.0), np.eye(3), 0.02)]
+    vol = synth.rasterise(ball, 32, 4.0).astype(np.float64)
+    for off in (0.0, 20.0):
+        g, _ = G(o, n_views=8, det_off_u_mm=off)
+        s = o.fp(g, vol)[0]
+        for i in range(8):
+            assert np.max(np.abs(s[i] - s[(i + 2) % 8])) < 1e-13
+        # neighbouring (45 deg) views differ: the invariance is not vacuous
+        assert np.max(np.abs(s[0] - s[1])) > 1e-3 * np.max(s)
+    # z-mirror symmetry of a z-symmetric phantom: rows flip
+    g, _ = G(o, n_views=3)
+    s = o.fp(g, vol)[0]
+    assert np.max(np.abs(s - s[:, ::-1, :])) < 1e-13
+
+
+def test_p7_all_ones_cube_axis_ray(oracle_mod):
+    """P7: zero-extension boundary rule R4: axis-parallel central ray through an
+    all-ones N^3 cube integrates to exactly N*h (ramps add h/2 each side)."""
+    o = oracle_mod
+    g, _ = G(o, vol_nx=8, vol_ny=8, vol_nz=8, det_nu=5, det_nv=5, n_views=4)
+    s = o.fp(g, np.ones((8, 8, 8)))[0]
+    for i in range(4):
+        assert abs(s[i, 2, 2] - 32.0) < 1e-12
+    # anisotropic grid size: view 0 runs along x, view 1 along y
+    g, _ = G(o, vol_nx=6, vol_ny=10, vol_nz=8, det_nu=5, det_nv=5, n_views=4)
+    s = o.fp(g, np.ones((8, 10, 6)))[0]
+    assert abs(s[0, 2, 2] - 24.0) < 1e-12 and abs(s[1, 2, 2] - 40.0) < 1e-12
+
+
+def test_p8_linearity_and_channels(oracle_mod):
+    o = oracle_mod
+    g, _ = G(o, n_views=5, det_off_u_mm=10.0)
+    rng = np.random.default_rng(3)
+    x = rng.normal(size=g.vol_shape(2))
+    s = o.fp(g, x)
+    assert np.max(np.abs(o.fp(g, 2.0 * x[0] - 3.0 * x[1])[0] - (2.0 * s[0] - 3.0 * s[1]))) < 1e-12
+    assert np.array_equal(o.fp(g, x[1])[0], s[1])
+    y = rng.normal(size=g.sino_shape(2))
+    b = o.bp_adjoint(g, y)
+    assert np.allclose(o.bp_adjoint(g, y[1])[0], b[1], rtol=0, atol=1e-13)
+    f = o.bp_fdk(g, y)
+    assert np.array_equal(o.bp_fdk(g, y[1])[0], f[1])
+
+
+def test_p9_slabs_and_clip(oracle_mod):
+    """P9: z-slabs sum to the whole (the lattice is anchored at the source, R3),
+    and the conservative k-clip drops no non-zero sample."""
+    o = oracle_mod
+    g, _ = G(o, n_views=5, det_off_u_mm=25.0, vol_cz_mm=6.0)
+    rng = np.random.default_rng(8)
+    x = rng.random(g.vol_shape(1))
+    full = o.fp(g, x, clip=True)
+    assert np.max(np.abs(full - o.fp(g, x, clip=False))) == 0.0
+    acc = np.zeros_like(full)
+    for z0 in range(0, 32, 11):
+        part = np.zeros_like(x)
+        part[:, z0:z0 + 11] = x[:, z0:z0 + 11]
+        acc += o.fp(g, part)
+    assert np.max(np.abs(acc - full)) < 1e-13
+    y = rng.random(g.sino_shape(1))
+    assert np.max(np.abs(o.bp_adjoint(g, y, clip=True) - o.bp_adjoint(g, y, clip=False))) < 1e-13
+    assert o.count_samples(g, clip=True) == o.count_samples(g, clip=False)
+
+
+def test_p10_strided_views(oracle_mod):
+    """P10 / R14: a geometry holding every 4th angle reproduces rows 0,4,8,..."""
+    o = oracle_mod
+    g, _ = G(o, n_views=12)
+    gs, _ = G(o, n_views=3, angles_rad=[2 * np.pi * i / 12 for i in (0, 4, 8)])
+    rng = np.random.default_rng(2)
+    x = rng.random(g.vol_shape(1))
+    assert np.array_equal(o.fp(g, x)[0, ::4], o.fp(gs, x)[0])
+
+
+def test_p11_fdk_weight_sum_closed_form(oracle_mod):
+    """P11: q == 1 on a wide detector: vol = n_views (1 - r^2/SID^2)^(-3/2)."""
+    o = oracle_mod
+    for nviews in (36, 90):
+        g, kw = G(o, n_views=nviews, det_nu=200, det_nv=200, vol_cx_mm=50.0, vol_cy_mm=-30.0)
+        vol = o.bp_fdk(g, np.ones(g.sino_shape(1)))[0]
+        ax = (np.arange(32) - 15.5) * 4.0
+        r2 = (ax[None, :] + 50.0) ** 2 + (ax[:, None] - 30.0) ** 2
+        ref = nviews * (1.0 - r2 / 1000.0 ** 2) ** (-1.5)
+        assert np.max(np.abs(vol - ref[None]) / ref[None]) < 1e-13
+
+
+def test_p11b_fdk_lands_on_projected_pixel(oracle_mod):
+    """A single lit detector pixel backprojects onto the voxels that project to
+    it (u*, v* mapping, bilinear weights, (SID/U)^2), checked by hand for one
+    voxel: pins the u/v order and signs in bp_fdk independently of fp."""
+    o = oracle_mod
+    g, kw = G(o, n_views=4, det_off_u_mm=8.0)
+    x, y, z = (20 - 15.5) * 4.0, (9 - 15.5) * 4.0, (25 - 15.5) * 4.0
+    for i in range(4):
+        phi = 2 * np.pi * i / 4
+        U = 1000.0 - (x * np.cos(phi) + y * np.sin(phi))
+        fu = (1536.0 * (-x * np.sin(phi) + y * np.cos(phi)) / U - 8.0) / 3.2 + 23.5
+        fv = (1536.0 * z / U) / 3.2 + 23.5
+        ju, jv = int(np.floor(fu)), int(np.floor(fv))
+        q = np.zeros(g.sino_shape(1))
+        q[0, i, jv + 1, ju] = 1.0
+        want = (1000.0 / U) ** 2 * (fv - jv) * (1.0 - (fu - ju))
+        got = o.bp_fdk(g, q)[0, 25, 9, 20]
+        assert abs(got - want) < 1e-13 and want > 0
+
+
+def test_p12_fdk_end_to_end_ball(oracle_mod):
+    """P12: cosine weight + ramp + (dphi/2) * bp_fdk reconstructs a ball's density."""
+    o = oracle_mod
+    nviews = 120
+    g, kw = G(o, n_views=nviews, det_nu=96, det_nv=64, det_du_mm=2.0, det_dv_mm=2.0,
+              vol_nx=24, vol_ny=24, vol_nz=8)
+    ball = [(np.zeros(3), np.full(3, 40.0), np.eye(3), 0.02)]
+    proj = an.ellipsoid_sinogram(kw, ball)
+    q = o.fdk_frontend(g, proj)
+    rec = (2 * np.pi / nviews / 2.0) * o.bp_fdk(g, q)[0]
+    ax = (np.arange(24) - 11.5) * 4.0
+    r = np.sqrt(ax[None, :] ** 2 + ax[:, None] ** 2)
+    mid = rec[4]                     # z = +2 mm plane
+    inside = mid[r < 30.0]
+    outside = mid[(r > 52.0)]
+    assert abs(np.mean(inside) - 0.02) < 2e-4, np.mean(inside)
+    assert np.max(np.abs(inside - 0.02)) < 8e-4
+    assert np.max(np.abs(outside)) < 1e-3
+
+
+def test_sampled_variants_match_full(oracle_mod):
+    """fp_rays / bp_adjoint_voxels / bp_fdk_voxels agree with the full operators
+    (pins the detector bounding-box pruning of bp_adjoint_voxels)."""
+    o = oracle_mod
+    g, _ = G(o, n_views=9, det_off_u_mm=40.0, vol_nx=20, vol_ny=18, vol_nz=14, det_nu=40, det_nv=30)
+    rng = np.random.default_rng(21)
+    x = rng.random(g.vol_shape(2))
+    y = rng.random(g.sino_shape(2))
+    ridx = synth.sample_indices(1, y[0].size, 300)
+    assert np.array_equal(o.fp_rays(g, x, ridx), o.fp(g, x).reshape(2, -1)[:, ridx])
+    vidx = np.concatenate([synth.sample_indices(2, x[0].size, 150), [0, x[0].size - 1]])
+    full = o.bp_adjoint(g, y).reshape(2, -1)[:, vidx]
+    part = o.bp_adjoint_voxels(g, y, vidx)
+    assert np.max(np.abs(full - part)) < 1e-12 * np.max(np.abs(full))
+    assert np.array_equal(o.bp_fdk_voxels(g, y, vidx), o.bp_fdk(g, y).reshape(2, -1)[:, vidx])
+
+
+def test_tiny_sample_count(oracle_mod):
+    """Tiny config in-support samples: ~68 per ray (32^3 box, 0.5-voxel step)."""
+    o = oracle_mod
+    g, _ = G(o)
+    n = o.count_samples(g)
+    rays = 36 * 48 * 48
+    assert 60.0 < n / rays < 75.0
