@@ -1,0 +1,287 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the cone-beam hot path on B200 (contract: see DESIGN.md s.8).
+
+One "step" = one pass of the whole hot path over one batch of synthetic input:
+cbct_fp + cbct_bp_adjoint + cbct_bp_fdk over all channels of the workload
+(default: BASELINE.json configs[3], the 8-channel 256^3 / 400-view primal-dual
+step).  `value` is the forward projector's Gsamples/s (in-support samples,
+counted analytically in fp64 by cbct_geom_count_samples); the backprojectors'
+Gvoxel-views/s are reported in `backprojection`.  All timing is CUDA events on
+the launching stream; inputs (1.3 GB) are larger than L2.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "forward Gsamples/s at 256^3 (backprojection Gvoxel-views/s in `backprojection`)"
+UNIT = "Gsamples/s"
+
+
+def peaks():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return json.load(f), "measured"
+    except Exception:
+        return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0}, "fallback"
+
+
+class ClockSampler:
+    """Samples nvidia-smi clocks / throttle reasons during the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.rows, self._stop, self._t = index, [], threading.Event(), None
+
+    def _run(self):
+        while not self._stop.is_set():
+            try:
+                out = subprocess.run(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                      "--format=csv,noheader,nounits"], capture_output=True, text=True, timeout=5)
+                if out.returncode == 0 and out.stdout.strip():
+                    self.rows.append([x.strip() for x in out.stdout.strip().split(",")])
+            except Exception:
+                pass
+            self._stop.wait(0.2)
+
+    def __enter__(self):
+        self._t = threading.Thread(target=self._run, daemon=True)
+        self._t.start()
+        return self
+
+    def __exit__(self, *a):
+        self._stop.set()
+        self._t.join(timeout=6)
+
+    def summary(self):
+        if not self.rows:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        sm = sorted(float(r[0]) for r in self.rows)
+        reasons = []
+        for k, name in ((3, "hw_slowdown"), (4, "hw_thermal_slowdown"), (5, "sw_thermal_slowdown"),
+                        (6, "sw_power_cap")):
+            if any(r[k].lower().startswith("active") for r in self.rows):
+                reasons.append(name)
+        return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": float(self.rows[0][1]),
+                "power_w_max": max(float(r[2]) for r in self.rows), "samples": len(self.rows), "reasons": reasons}
+
+
+def oracle_sample(cfg, steps, warmup):
+    """The fp64 oracle, as it stands, on a bounded sample of the workload:
+    channel 0, every 16th view, forward projection (Gsamples/s)."""
+    import numpy as np
+    import oracle
+    from paper_2512_21180_b200 import synth
+    kw = synth.geom_kwargs(cfg)
+    stride = 16 if cfg["n_views"] >= 64 else 1
+    views = list(range(0, cfg["n_views"], stride))
+    sub = dict(kw, n_views=len(views))
+    og = oracle.Geom(**sub, angles_rad=[2 * np.pi * i / cfg["n_views"] for i in views])
+    vol = synth.make_volume(cfg, channels=1).astype(np.float64)
+    nsamp = oracle.count_samples(og)
+    times = []
+    for it in range(warmup + steps):
+        t0 = time.perf_counter()
+        oracle.fp(og, vol)
+        if it >= warmup:
+            times.append(time.perf_counter() - t0)
+    dt = sum(times) / len(times)
+    return {"value": nsamp / dt / 1e9, "unit": UNIT, "cores": oracle.max_threads(), "kind": "oracle",
+            "sample": f"cbct_fp of channel 0, {len(views)} of {cfg['n_views']} views (every {stride}th), "
+                      f"{nsamp:.3e} samples, {dt:.2f} s per pass"}, dt
+
+
+def run_reference(args, cfg):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    cb, dt = oracle_sample(cfg, max(1, min(args.steps, 3)), min(args.warmup, 1))
+    line = {"impl": "reference", "metric": METRIC, "value": cb["value"], "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": cfg["name"], "note": "oracle on host cores, bounded sample"},
+            "cpu_baseline": cb,
+            "e2e": {"value": cb["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="multichannel_256")
+    ap.add_argument("--channels", type=int, default=0, help="override the workload's channel count")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    args = ap.parse_args()
+
+    from paper_2512_21180_b200 import synth
+    cfg = dict(synth.CONFIGS[args.workload])
+    if args.channels:
+        cfg["channels"] = args.channels
+    if args.impl == "reference":
+        run_reference(args, cfg)
+        return
+
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    from paper_2512_21180_b200 import cbct
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    C = cfg["channels"]
+    kw = synth.geom_kwargs(cfg)
+    g = cbct.Geometry(**kw)
+    n_samples = g.count_samples()                    # per channel, analytic fp64 (host)
+    n_vv = g.n_vol * cfg["n_views"]                  # voxel-views per channel
+    # every rank works on its own batch of C channels (weak scaling, no data-path collective)
+    vol_h = synth.make_volume(cfg)
+    sino_h = synth.make_sinogram(cfg)
+    vol = torch.from_numpy(vol_h).cuda()
+    sino_in = torch.from_numpy(sino_h).cuda()
+    sino_out = torch.empty_like(sino_in)
+    vol_out = torch.empty_like(vol)
+
+    def step(ev=None):
+        if ev:
+            ev[0].record()
+        g.fp(vol, sino_out, C)
+        if ev:
+            ev[1].record()
+        g.bp_adjoint(sino_in, vol_out, C)
+        if ev:
+            ev[2].record()
+        g.bp_fdk(sino_in, vol_out, C)
+        if ev:
+            ev[3].record()
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        step()
+    barrier()
+    l0 = g.launch_count()
+    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(4)] for _ in range(args.steps)]
+    with ClockSampler(local) as clk:
+        for k in range(args.steps):
+            step(evs[k])
+        barrier()
+    launches = g.launch_count() - l0
+    t_fp = sum(e[0].elapsed_time(e[1]) for e in evs) / args.steps
+    t_adj = sum(e[1].elapsed_time(e[2]) for e in evs) / args.steps
+    t_fdk = sum(e[2].elapsed_time(e[3]) for e in evs) / args.steps
+    t_total = evs[0][0].elapsed_time(evs[-1][3]) / args.steps
+    tt = torch.tensor([t_fp, t_adj, t_fdk, t_total], device="cuda", dtype=torch.float64)
+    if world > 1:
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+    t_fp, t_adj, t_fdk, t_total = [float(x) for x in tt.cpu()]
+
+    # end to end through the C ABI with HOST (pinned) buffers: copies inside the timed region
+    e2e = None
+    if not args.no_e2e:
+        hv, hs = torch.from_numpy(vol_h).pin_memory(), torch.from_numpy(sino_h).pin_memory()
+        hso, hvo = torch.empty_like(hs).pin_memory(), torch.empty_like(hv).pin_memory()
+        def e2e_step(ev=None):
+            if ev:
+                ev[0].record()
+            g.fp(hv, hso, C)
+            if ev:
+                ev[1].record()
+            g.bp_adjoint(hs, hvo, C)
+            g.bp_fdk(hs, hvo, C)
+            if ev:
+                ev[2].record()
+        e2e_step()
+        barrier()
+        ev2 = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(args.steps)]
+        for k in range(args.steps):
+            e2e_step(ev2[k])
+        barrier()
+        te = torch.tensor([sum(e[0].elapsed_time(e[1]) for e in ev2) / args.steps,
+                           ev2[0][0].elapsed_time(ev2[-1][2]) / args.steps], device="cuda", dtype=torch.float64)
+        if world > 1:
+            dist.all_reduce(te, op=dist.ReduceOp.MAX)
+        te_fp, te_step = [float(x) for x in te.cpu()]
+        e2e = {"value": world * C * n_samples / (te_fp * 1e-3) / 1e9, "unit": UNIT,
+               "h2d_bytes_per_step": int(vol_h.nbytes + 2 * sino_h.nbytes),
+               "d2h_bytes_per_step": int(sino_h.nbytes + 2 * vol_h.nbytes),
+               "ms_per_step": te_step, "fp_ms": te_fp,
+               "note": "cbct_fp/bp_adjoint/bp_fdk called with pinned HOST buffers; value = forward Gsamples/s incl. copies"}
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    pk, pk_src = peaks()
+    clocks = clk.summary()
+    sm_hz = (clocks["sm_mhz"] or pk.get("sm_max_mhz", 1965.0)) * 1e6
+    fwd = world * C * n_samples / (t_fp * 1e-3) / 1e9
+    adj_vv = world * C * n_vv / (t_adj * 1e-3) / 1e9
+    fdk_vv = world * C * n_vv / (t_fdk * 1e-3) / 1e9
+    # roofline of the dominant call (see DESIGN.md s.7): algorithmic on-SM tap bytes
+    # per unit (fp 32 B/sample, adjoint 64 B/sample, fdk 16 B/voxel-view) against
+    # 148 SMs x 128 B/clk at the SM clock seen under load.
+    l1_peak = 148 * 128 * sm_hz / 1e9
+    calls = {"cbct_fp": (t_fp, 32.0 * C * n_samples), "cbct_bp_adjoint": (t_adj, 64.0 * C * n_samples),
+             "cbct_bp_fdk": (t_fdk, 16.0 * C * n_vv)}
+    dom = max(calls, key=lambda k: calls[k][0])
+    ach = calls[dom][1] / (calls[dom][0] * 1e-3) / 1e9
+    hbm_bytes = {"cbct_fp": C * 4.0 * (g.n_vol + g.n_sino), "cbct_bp_adjoint": C * 4.0 * (g.n_vol + g.n_sino),
+                 "cbct_bp_fdk": C * 4.0 * (g.n_vol + g.n_sino)}
+    roofline = {"kernel": dom, "bound": "l1", "achieved": ach, "peak": l1_peak, "unit": "GB/s",
+                "frac": ach / l1_peak, "traffic": None,
+                "peak_source": f"148 SM x 128 B/clk x {sm_hz / 1e6:.0f} MHz (on-SM L1/shared pipe; "
+                               "HBM is not the bound: see hbm_frac)",
+                "hbm_frac": hbm_bytes[dom] / (calls[dom][0] * 1e-3) / 1e9 / pk["hbm_gbs"],
+                "hbm_peak_source": pk_src,
+                "per_call": {k: {"ms": v[0], "l1_frac": v[1] / (v[0] * 1e-3) / 1e9 / l1_peak} for k, v in calls.items()}}
+    line = {"metric": METRIC, "value": fwd, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": t_total, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": cfg["name"], "volume": [cfg["vol_nz"], cfg["vol_ny"], cfg["vol_nx"]],
+                       "vox_mm": cfg["vox_mm"], "views": cfg["n_views"], "detector": [cfg["det_nv"], cfg["det_nu"]],
+                       "channels": C, "step_vox": cfg["step_vox"], "l2": "inputs larger than L2 (no flush)",
+                       "sharding": "each rank runs its own C-channel batch; no data-path collective"},
+            "backprojection": {"adjoint_gvoxel_views_per_s": adj_vv, "adjoint_gsamples_per_s":
+                               world * C * n_samples / (t_adj * 1e-3) / 1e9,
+                               "fdk_gvoxel_views_per_s": fdk_vv, "unit": "Gvoxel-views/s"},
+            "call_ms": {"cbct_fp": t_fp, "cbct_bp_adjoint": t_adj, "cbct_bp_fdk": t_fdk},
+            "samples_per_channel": n_samples, "voxel_views_per_channel": n_vv,
+            "gpu_launches": int(launches), "clocks": clocks, "roofline": roofline}
+    if e2e:
+        line["e2e"] = e2e
+    if not args.no_cpu_baseline and world == 1:
+        line["cpu_baseline"], _ = oracle_sample(cfg, 1, 0)
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,139 @@
+/*
+ * cbct.h -- C ABI of libcbct.so: circular-orbit cone-beam CT operators for
+ * NVIDIA B200 (sm_100a), the data-parallel hot path of LIRE++
+ * (arxiv 2512.21180; section/line citations refer to PAPER.md).
+ *
+ *   P   forward projector   PAPER.md:85-89 Eq. (5): P(mu)(t,u) = int_{L_{t,u}} mu(z) dz,
+ *                           L_{t,u} the line from the source to detector element u at view t
+ *   P*  backprojector       PAPER.md:89 (+ footnote :101): the Hermitian adjoint of P
+ *   FDK backprojection      PAPER.md:157, :181 (Alg. 1 l.3), ref [9] :397 (Feldkamp)
+ *   geometry                PAPER.md:61 (SID 1000 mm, isocentre-detector 536 mm,
+ *                           115 mm lateral detector offset, 409.6 mm / 256^2 panel)
+ *   multi-channel use       PAPER.md:167, :221, :227, :230 (Alg. 1 l.16-19)
+ *   multi-scale use         PAPER.md:270 (one handle per scale / view subset)
+ *   streaming               PAPER.md:165, :292 (data kept on the host, parts sent to the GPU)
+ *
+ * The paper defines P only as a continuous integral; the discretisation is
+ * the one BASELINE.json names (ray-driven, trilinear samples at a fixed step)
+ * with the readings R1-R11 listed in DESIGN.md section 3.
+ *
+ * Conventions
+ *   - World frame (mm): isocentre at the origin, rotation axis +z.  View i has
+ *     angle phi_i; source s_i = SID (cos phi_i, sin phi_i, 0); detector centre
+ *     -(SDD-SID)(cos phi_i, sin phi_i, 0); e_u = (-sin phi_i, cos phi_i, 0),
+ *     e_v = (0,0,1).  Pixel (iv,iu) centre: u = (iu-(nu-1)/2) du + off_u,
+ *     v = (iv-(nv-1)/2) dv + off_v.
+ *   - Volume: voxel (iz,iy,ix) centre at c + (i-(N-1)/2) h per axis; zero
+ *     outside the grid, trilinear interpolation fades to zero over the outer
+ *     voxel (support -1 < q < N in index coordinates).
+ *   - Layouts (fp32, C-contiguous): vol[C][nz][ny][nx] (x fastest),
+ *     sino[C][n_views][nv][nu] (u fastest).
+ *   - Every data pointer may be a DEVICE pointer or a HOST pointer (pinned or
+ *     pageable); the library detects which with cudaPointerGetAttributes.
+ *     Host buffers are staged through library-owned device workspace inside
+ *     the call (copies are enqueued on `cuda_stream`; a call with any pageable
+ *     host buffer synchronises the stream before returning).
+ *   - Outputs are OVERWRITTEN, never accumulated into.
+ *   - Ownership: the caller owns all data buffers; the library owns the
+ *     handle and its device workspace, freed by cbct_geom_destroy.
+ *   - Asynchrony: with device pointers all work is enqueued on `cuda_stream`
+ *     (a cudaStream_t cast to void*, NULL = legacy default stream) and the
+ *     call returns without synchronising.  A handle carries mutable
+ *     workspace: calls on one handle must be ordered on one stream at a time.
+ *   - Errors: 0 on success, a negative cbct_status otherwise; nothing throws
+ *     across the ABI.  There is NO CPU fallback: without a CUDA device every
+ *     compute entry point returns CBCT_ERR_CUDA.
+ */
+#ifndef CBCT_H
+#define CBCT_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum cbct_status {
+    CBCT_OK = 0,
+    CBCT_ERR_INVALID_ARG = -1, /* NULL pointer, non-positive size, geometry that puts samples
+                                  behind the source or beyond the detector, bad step      */
+    CBCT_ERR_UNSUPPORTED = -2, /* e.g. more views than CBCT_MAX_VIEWS                      */
+    CBCT_ERR_CUDA = -3,        /* a CUDA runtime call failed (cbct_last_cuda_error)        */
+    CBCT_ERR_NOMEM = -4        /* host or device allocation failed, or the work-set cap
+                                  is too small for even one slab                           */
+} cbct_status;
+
+#define CBCT_MAX_VIEWS 4096
+
+typedef struct cbct_geom cbct_geom; /* opaque; owns host tables + device workspace */
+
+/* Geometry descriptor (host memory, copied at create time).  Defaults of the
+ * paper's scanner in comments. */
+typedef struct cbct_geom_desc {
+    double sid_mm;                /* source-isocentre distance                 1000       */
+    double sdd_mm;                /* source-detector distance                  1536       */
+    int32_t n_views;              /* 1..CBCT_MAX_VIEWS                         400..944   */
+    const double *angles_rad;     /* n_views angles, or NULL => 2*pi*i/n_views            */
+    int32_t det_nu, det_nv;       /* detector columns (lateral u), rows (axial v)  256    */
+    double det_du_mm, det_dv_mm;  /* pixel pitch                               1.6        */
+    double det_off_u_mm;          /* lateral offset along e_u (half-fan)       +115       */
+    double det_off_v_mm;          /* axial offset along e_v                    0          */
+    int32_t vol_nx, vol_ny, vol_nz; /* grid size                               256^3      */
+    double vox_mm;                /* isotropic voxel pitch h                   2.0        */
+    double vol_cx_mm, vol_cy_mm, vol_cz_mm; /* volume centre rel. to isocentre  0,0,0     */
+    double step_vox;              /* ray step in voxel units, 0 < step <= 1    0.5        */
+    uint64_t max_workset_bytes;   /* 0 = no cap; else cap on device bytes holding volume
+                                     data at once => z-slab streaming (A5)               */
+} cbct_geom_desc;
+
+/* A1.  Validates `d`, precomputes the per-view tables (fp64 on the host,
+ * passed to the kernels through constant memory) and returns a handle in
+ * *out.  Needs no CUDA device (device workspace is allocated lazily by the
+ * first compute call).  Requires sdd > sid, the sphere bounding the
+ * zero-extended volume strictly between source and detector plane, positive
+ * sizes and pitches, 0 < step_vox <= 1. */
+int cbct_geom_create(const cbct_geom_desc *d, cbct_geom **out);
+
+/* Frees the handle, its tables and its device workspace (synchronises the device). */
+int cbct_geom_destroy(cbct_geom *g);
+
+/* A2.  sino[c,i,iv,iu] = Delta * sum_k T[vol_c](q(s_i + t_k d)),  t_k = (k+1/2) Delta,
+ * Delta = step_vox * vox_mm, k over all samples between source and pixel, T the
+ * zero-extended trilinear interpolant, d the unit vector source -> pixel centre.
+ * vol: channels*nz*ny*nx floats (read), sino: channels*n_views*nv*nu floats (written). */
+int cbct_fp(const cbct_geom *g, const float *vol, float *sino, int32_t channels, void *cuda_stream);
+
+/* A3.  The exact transpose of the matrix applied by cbct_fp (plain Euclidean
+ * dot products): vol_c[j] = Delta * sum_{i,iv,iu,k} w(j; i,iv,iu,k) sino_c[i,iv,iu].
+ * Floating-point summation order is unspecified (fp32 accumulation). */
+int cbct_bp_adjoint(const cbct_geom *g, const float *sino, float *vol, int32_t channels, void *cuda_stream);
+
+/* A4.  Backprojection stage of FDK for a flat detector, voxel-driven:
+ * vol_c[z,y,x] = sum_i (SID/U_i)^2 * B[sino_c,i](fv, fu),  U_i = SID - (x cos phi_i + y sin phi_i),
+ * u* = SDD (-x sin phi_i + y cos phi_i)/U_i, v* = SDD z/U_i, (fu,fv) their detector index
+ * coordinates, B the zero-extended bilinear interpolant.  `sino` is the already
+ * weighted + ramp-filtered projection data; no dphi/2 factor is applied. */
+int cbct_bp_fdk(const cbct_geom *g, const float *sino, float *vol, int32_t channels, void *cuda_stream);
+
+/* Number of in-support samples of ONE channel: pairs (ray, k) with -1 < q < N
+ * on every axis, counted analytically in fp64 on the host from the geometry
+ * (the unit of the forward Gsamples/s metric).  Needs no CUDA device. */
+int cbct_geom_count_samples(const cbct_geom *g, uint64_t *out);
+
+/* Number of z-slabs the streaming path (A5) uses for `channels` channels
+ * (1 = everything resident).  Needs no CUDA device. */
+int cbct_geom_num_slabs(const cbct_geom *g, int32_t channels, int32_t *out);
+
+/* Kernels launched by this handle since creation (for bench.py's gpu_launches). */
+int cbct_geom_launch_count(const cbct_geom *g, uint64_t *out);
+
+/* Static description of a status code. */
+const char *cbct_status_string(int status);
+
+/* Text of the last CUDA error seen by the calling thread ("" if none). */
+const char *cbct_last_cuda_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CBCT_H */

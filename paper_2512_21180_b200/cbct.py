@@ -1,0 +1,185 @@
+"""Thin ctypes binding over the C ABI of libcbct.so (include/cbct.h).
+
+Argument marshalling only: every step of the hot path runs in the CUDA
+kernels behind `cbct_fp`, `cbct_bp_adjoint`, `cbct_bp_fdk`.  There is no CPU
+fallback: if libcbct.so is missing, or no CUDA device is present, calls raise.
+Tensors may be torch CUDA tensors, torch CPU tensors (pinned or not) or numpy
+arrays, fp32 and C-contiguous; PyTorch is used for memory and streams only.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import Optional, Sequence
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libcbct.so")
+
+EXPORTS = (
+    "cbct_geom_create", "cbct_geom_destroy", "cbct_fp", "cbct_bp_adjoint", "cbct_bp_fdk",
+    "cbct_geom_count_samples", "cbct_geom_num_slabs", "cbct_geom_launch_count",
+    "cbct_status_string", "cbct_last_cuda_error",
+)
+
+
+class CbctError(RuntimeError):
+    pass
+
+
+class GeomDesc(ctypes.Structure):
+    """struct cbct_geom_desc (include/cbct.h)."""
+    _fields_ = [
+        ("sid_mm", ctypes.c_double), ("sdd_mm", ctypes.c_double),
+        ("n_views", ctypes.c_int32),
+        ("angles_rad", ctypes.POINTER(ctypes.c_double)),
+        ("det_nu", ctypes.c_int32), ("det_nv", ctypes.c_int32),
+        ("det_du_mm", ctypes.c_double), ("det_dv_mm", ctypes.c_double),
+        ("det_off_u_mm", ctypes.c_double), ("det_off_v_mm", ctypes.c_double),
+        ("vol_nx", ctypes.c_int32), ("vol_ny", ctypes.c_int32), ("vol_nz", ctypes.c_int32),
+        ("vox_mm", ctypes.c_double),
+        ("vol_cx_mm", ctypes.c_double), ("vol_cy_mm", ctypes.c_double), ("vol_cz_mm", ctypes.c_double),
+        ("step_vox", ctypes.c_double),
+        ("max_workset_bytes", ctypes.c_uint64),
+    ]
+
+
+_lib = None
+
+
+def load_library() -> ctypes.CDLL:
+    """Load libcbct.so (built in-tree by paper_2512_21180_b200/build.py).  Fails loudly."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise CbctError(
+            f"{LIB_PATH} is missing: build it with `python -m paper_2512_21180_b200.build` "
+            "(or __graft_entry__.build()); there is no CPU fallback")
+    L = ctypes.CDLL(LIB_PATH)
+    vp, i32 = ctypes.c_void_p, ctypes.c_int32
+    L.cbct_geom_create.argtypes = [ctypes.POINTER(GeomDesc), ctypes.POINTER(vp)]
+    L.cbct_geom_destroy.argtypes = [vp]
+    for name in ("cbct_fp", "cbct_bp_adjoint", "cbct_bp_fdk"):
+        getattr(L, name).argtypes = [vp, vp, vp, i32, vp]
+    L.cbct_geom_count_samples.argtypes = [vp, ctypes.POINTER(ctypes.c_uint64)]
+    L.cbct_geom_num_slabs.argtypes = [vp, i32, ctypes.POINTER(i32)]
+    L.cbct_geom_launch_count.argtypes = [vp, ctypes.POINTER(ctypes.c_uint64)]
+    L.cbct_status_string.argtypes = [ctypes.c_int]
+    L.cbct_status_string.restype = ctypes.c_char_p
+    L.cbct_last_cuda_error.restype = ctypes.c_char_p
+    _lib = L
+    return L
+
+
+def _check(rc: int):
+    if rc != 0:
+        L = load_library()
+        msg = L.cbct_status_string(rc).decode()
+        cuda = L.cbct_last_cuda_error().decode()
+        raise CbctError(f"{msg}" + (f" [{cuda}]" if cuda and rc == -3 else ""))
+
+
+def _ptr_and_keep(t, n_expected: int):
+    """Raw address of an fp32 contiguous torch tensor / numpy array."""
+    if isinstance(t, np.ndarray):
+        if t.dtype != np.float32 or not t.flags["C_CONTIGUOUS"]:
+            raise CbctError("numpy buffers must be float32 and C-contiguous")
+        if t.size != n_expected:
+            raise CbctError(f"buffer has {t.size} elements, expected {n_expected}")
+        return t.ctypes.data
+    import torch
+    if not isinstance(t, torch.Tensor):
+        raise CbctError("expected a torch.Tensor or numpy.ndarray")
+    if t.dtype != torch.float32 or not t.is_contiguous():
+        raise CbctError("tensors must be float32 and contiguous")
+    if t.numel() != n_expected:
+        raise CbctError(f"tensor has {t.numel()} elements, expected {n_expected}")
+    return t.data_ptr()
+
+
+def _stream_handle(stream) -> int:
+    if stream is None:
+        import torch
+        if torch.cuda.is_available():
+            return int(torch.cuda.current_stream().cuda_stream)
+        return 0
+    if isinstance(stream, int):
+        return stream
+    return int(stream.cuda_stream)
+
+
+class Geometry:
+    """Owns one `cbct_geom*` handle (A1, `cbct_geom_create`)."""
+
+    def __init__(self, *, sid_mm=1000.0, sdd_mm=1536.0, n_views, det_nu, det_nv, det_du_mm, det_dv_mm,
+                 det_off_u_mm=0.0, det_off_v_mm=0.0, vol_nx, vol_ny, vol_nz, vox_mm,
+                 vol_cx_mm=0.0, vol_cy_mm=0.0, vol_cz_mm=0.0, step_vox=0.5,
+                 angles_rad: Optional[Sequence[float]] = None, max_workset_bytes: int = 0):
+        L = load_library()
+        d = GeomDesc()
+        d.sid_mm, d.sdd_mm, d.n_views = sid_mm, sdd_mm, n_views
+        d.det_nu, d.det_nv, d.det_du_mm, d.det_dv_mm = det_nu, det_nv, det_du_mm, det_dv_mm
+        d.det_off_u_mm, d.det_off_v_mm = det_off_u_mm, det_off_v_mm
+        d.vol_nx, d.vol_ny, d.vol_nz, d.vox_mm = vol_nx, vol_ny, vol_nz, vox_mm
+        d.vol_cx_mm, d.vol_cy_mm, d.vol_cz_mm = vol_cx_mm, vol_cy_mm, vol_cz_mm
+        d.step_vox, d.max_workset_bytes = step_vox, int(max_workset_bytes)
+        if angles_rad is not None:
+            a = np.ascontiguousarray(np.asarray(angles_rad, dtype=np.float64))
+            if a.shape != (n_views,):
+                raise CbctError("angles_rad must have n_views entries")
+            d.angles_rad = a.ctypes.data_as(ctypes.POINTER(ctypes.c_double))
+        self.desc = d
+        self._h = ctypes.c_void_p()
+        _check(L.cbct_geom_create(ctypes.byref(d), ctypes.byref(self._h)))
+        self.n_vol = vol_nx * vol_ny * vol_nz
+        self.n_sino = n_views * det_nv * det_nu
+        self.vol_shape = (vol_nz, vol_ny, vol_nx)
+        self.sino_shape = (n_views, det_nv, det_nu)
+
+    def close(self):
+        if getattr(self, "_h", None) and self._h.value:
+            load_library().cbct_geom_destroy(self._h)
+            self._h = ctypes.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # --- the hot path -------------------------------------------------------
+    def fp(self, vol, sino, channels: int = 1, stream=None):
+        """cbct_fp: vol[C,nz,ny,nx] -> sino[C,n_views,nv,nu] (overwritten)."""
+        pv, ps = _ptr_and_keep(vol, channels * self.n_vol), _ptr_and_keep(sino, channels * self.n_sino)
+        _check(load_library().cbct_fp(self._h, pv, ps, channels, _stream_handle(stream)))
+        return sino
+
+    def bp_adjoint(self, sino, vol, channels: int = 1, stream=None):
+        """cbct_bp_adjoint: sino -> vol (overwritten), exact transpose of fp."""
+        ps, pv = _ptr_and_keep(sino, channels * self.n_sino), _ptr_and_keep(vol, channels * self.n_vol)
+        _check(load_library().cbct_bp_adjoint(self._h, ps, pv, channels, _stream_handle(stream)))
+        return vol
+
+    def bp_fdk(self, sino, vol, channels: int = 1, stream=None):
+        """cbct_bp_fdk: FDK-weighted voxel-driven backprojection stage."""
+        ps, pv = _ptr_and_keep(sino, channels * self.n_sino), _ptr_and_keep(vol, channels * self.n_vol)
+        _check(load_library().cbct_bp_fdk(self._h, ps, pv, channels, _stream_handle(stream)))
+        return vol
+
+    # --- host-side queries --------------------------------------------------
+    def count_samples(self) -> int:
+        out = ctypes.c_uint64()
+        _check(load_library().cbct_geom_count_samples(self._h, ctypes.byref(out)))
+        return int(out.value)
+
+    def num_slabs(self, channels: int = 1) -> int:
+        out = ctypes.c_int32()
+        _check(load_library().cbct_geom_num_slabs(self._h, channels, ctypes.byref(out)))
+        return int(out.value)
+
+    def launch_count(self) -> int:
+        out = ctypes.c_uint64()
+        _check(load_library().cbct_geom_launch_count(self._h, ctypes.byref(out)))
+        return int(out.value)

@@ -1,0 +1,96 @@
+// cbct_internal.h -- shared declarations of libcbct.so (product code; no oracle code).
+//
+// Coordinates used by every kernel: "voxel units" = world mm / vox_mm, world
+// origin at the isocentre.  A device volume buffer ("padded
+// volume") holds planes [z0, z1) of the grid with a zero border of CBCT_PAD
+// voxels on every side, so the zero-extended trilinear interpolant (reading
+// R4, DESIGN.md s.3) needs no bounds test in the sample loop:
+//     padded index p = q + CBCT_PAD  (z: q - z0 + CBCT_PAD).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <vector>
+
+#include "../../include/cbct.h"
+
+#define CBCT_PAD 2              // zero border (voxels / pixels) of padded buffers
+#define CBCT_VIEWS_PER_LAUNCH 512
+
+// View-independent geometry in voxel units (fp64), passed by value to kernels.
+struct RayGeom {
+    double sid, idd;        // source-isocentre, isocentre-detector distance
+    double u0, du, v0, dv;  // detector coordinate of pixel 0 and pixel pitch
+    double cx, cy, cz;      // volume centre
+    double step;            // ray step (voxel units)
+    double delta;           // ray step in mm = step * vox_mm (scale of the line integral)
+    int nu, nv;             // detector size
+    int nx, ny, nz;         // full grid size
+    int z0, z1;             // planes [z0, z1) held by the padded buffer
+    int px, py, pz;         // padded buffer dims (x pitch, rows, planes)
+};
+
+struct ViewChunk {
+    double2 cs[CBCT_VIEWS_PER_LAUNCH];  // (cos phi, sin phi)
+};
+
+// fp32 per-launch parameters of the FDK backprojection kernel.
+struct FdkGeom {
+    float sid;              // voxel units
+    float au, bu, av, bv;   // fu_pad = au * (-X s + Y c) / U + bu ; fv_pad = av * Z / U + bv
+    float x0, y0, z0;       // centred world coordinate (voxel units) of voxel index 0
+    float fu_max, fv_max;   // clamp range upper bounds in padded pixel coordinates
+    int nx, ny, nz;
+    int zs0, zs1;           // z planes [zs0, zs1) written by this launch
+    int pu, pv;             // padded sinogram pitch / rows
+    int n_views;
+};
+
+struct cbct_geom {
+    cbct_geom_desc d;
+    std::vector<double> angles, cosphi, sinphi;
+    // device workspace (lazily allocated, grown on demand)
+    float *ws_vol = nullptr;   size_t ws_vol_bytes = 0;    // padded volume(s)
+    float *ws_sino = nullptr;  size_t ws_sino_bytes = 0;   // padded / staged sinogram
+    float *ws_stage = nullptr; size_t ws_stage_bytes = 0;  // staging of host buffers
+    cudaStream_t copy_stream = nullptr;
+    cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
+    uint64_t launches = 0;
+    int64_t sample_count = -1;
+};
+
+void cbct_set_cuda_error(cudaError_t e, const char *what);
+
+#define CBCT_CUDA_TRY(expr)                                 \
+    do {                                                    \
+        cudaError_t e__ = (expr);                           \
+        if (e__ != cudaSuccess) {                           \
+            cbct_set_cuda_error(e__, #expr);                \
+            return CBCT_ERR_CUDA;                           \
+        }                                                   \
+    } while (0)
+
+// --- geometry helpers (cbct_geom.cu) ---------------------------------------
+RayGeom cbct_make_raygeom(const cbct_geom *g, int z0, int z1);
+size_t cbct_padded_volume_elems(const RayGeom &r);  // per channel
+int cbct_padded_sino_pitch(const cbct_geom *g);
+int cbct_padded_sino_rows(const cbct_geom *g);
+int cbct_plan_slab_planes(const cbct_geom *g, int channels);  // planes per z-slab, <1 = cap too small
+
+// --- kernel launchers (cbct_kernels.cu); all enqueue on `st` ----------------
+// pad:   src[C][nz_src][ny][nx] planes [z0,z1) -> dst[C][pz][py][px] (zero border)
+int cbct_launch_pad_volume(cbct_geom *g, const RayGeom &r, const float *src, float *dst, int channels,
+                           size_t src_channel_stride, int src_z_origin, cudaStream_t st);
+// unpad: padded dst planes -> vol[C][..] planes [z0,z1)
+int cbct_launch_unpad_volume(cbct_geom *g, const RayGeom &r, const float *padded, float *dst, int channels,
+                             size_t dst_channel_stride, int dst_z_origin, cudaStream_t st);
+int cbct_launch_pad_sino(cbct_geom *g, const float *src, float *dst, int channels, cudaStream_t st);
+// forward projection of the padded volume(s); accumulate != 0 adds into sino
+int cbct_launch_fp(cbct_geom *g, const RayGeom &r, const float *padded, float *sino, int channels,
+                   int accumulate, cudaStream_t st);
+// adjoint scatter into zeroed padded volume(s)
+int cbct_launch_adjoint(cbct_geom *g, const RayGeom &r, const float *sino, float *padded, int channels,
+                        cudaStream_t st);
+// FDK backprojection from the padded sinogram into vol planes [zs0, zs1)
+int cbct_launch_fdk(cbct_geom *g, const float *padded_sino, float *vol, int channels, int zs0, int zs1,
+                    size_t vol_channel_stride, int vol_z_origin, cudaStream_t st);

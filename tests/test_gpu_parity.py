@@ -1,0 +1,244 @@
+"""GPU parity: CUDA path (through the C ABI) vs the fp64 oracle, element by
+element on the same seeded inputs.  Tolerances are BASELINE.json's:
+forward / FDK rel-L2 <= 1e-5 and max-rel <= 1e-4, adjoint rel-L2 <= 1e-4,
+fp32 adjoint identity <= 1e-5 (norm definitions: reading R16, DESIGN.md s.3).
+"""
+import numpy as np
+import pytest
+
+from paper_2512_21180_b200 import synth
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+
+@pytest.fixture(scope="module")
+def cbct():
+    if not torch.cuda.is_available():
+        pytest.fail("gpu-marked tests need a CUDA device (no CPU fallback exists)")
+    from paper_2512_21180_b200 import cbct as m
+    m.load_library()
+    return m
+
+
+def rel_l2(g, r):
+    return float(np.linalg.norm((g - r).ravel()) / np.linalg.norm(r.ravel()))
+
+
+def max_rel(g, r):
+    """max |g-r| / max(|r|, 1e-3 * max|r|)  (R16)."""
+    floor = 1e-3 * float(np.max(np.abs(r)))
+    return float(np.max(np.abs(g - r) / np.maximum(np.abs(r), floor)))
+
+
+def dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def run_fp(m, kw, vol, **extra):
+    g = m.Geometry(**kw, **extra)
+    C = vol.shape[0]
+    out = torch.full((C,) + g.sino_shape, float("nan"), device="cuda", dtype=torch.float32)
+    g.fp(dev(vol), out, C)
+    torch.cuda.synchronize()
+    return out.cpu().numpy().astype(np.float64)
+
+
+def run_adj(m, kw, sino, **extra):
+    g = m.Geometry(**kw, **extra)
+    C = sino.shape[0]
+    out = torch.full((C,) + g.vol_shape, float("nan"), device="cuda", dtype=torch.float32)
+    g.bp_adjoint(dev(sino), out, C)
+    torch.cuda.synchronize()
+    return out.cpu().numpy().astype(np.float64)
+
+
+def run_fdk(m, kw, sino, **extra):
+    g = m.Geometry(**kw, **extra)
+    C = sino.shape[0]
+    out = torch.full((C,) + g.vol_shape, float("nan"), device="cuda", dtype=torch.float32)
+    g.bp_fdk(dev(sino), out, C)
+    torch.cuda.synchronize()
+    return out.cpu().numpy().astype(np.float64)
+
+
+def check_all_three(m, o, kw, vol, sino, tag=""):
+    og = o.Geom(**kw)
+    r = o.fp(og, vol.astype(np.float64))
+    g = run_fp(m, kw, vol)
+    assert rel_l2(g, r) <= 1e-5, (tag, "fp rel-L2", rel_l2(g, r))
+    assert max_rel(g, r) <= 1e-4, (tag, "fp max-rel", max_rel(g, r))
+    r = o.bp_adjoint(og, sino.astype(np.float64))
+    g = run_adj(m, kw, sino)
+    assert rel_l2(g, r) <= 1e-4, (tag, "adjoint rel-L2", rel_l2(g, r))
+    r = o.bp_fdk(og, sino.astype(np.float64))
+    g = run_fdk(m, kw, sino)
+    assert rel_l2(g, r) <= 1e-5, (tag, "fdk rel-L2", rel_l2(g, r))
+    assert max_rel(g, r) <= 1e-4, (tag, "fdk max-rel", max_rel(g, r))
+
+
+def test_config1_tiny(cbct, oracle_mod):
+    cfg = synth.CONFIGS["tiny"]
+    check_all_three(cbct, oracle_mod, synth.geom_kwargs(cfg), synth.make_volume(cfg), synth.make_sinogram(cfg), "tiny")
+
+
+def test_config2_small_halffan(cbct, oracle_mod):
+    cfg = synth.CONFIGS["small_halffan"]
+    check_all_three(cbct, oracle_mod, synth.geom_kwargs(cfg), synth.make_volume(cfg), synth.make_sinogram(cfg),
+                    "small")
+
+
+def test_ragged_sizes_offcentre_multichannel(cbct, oracle_mod):
+    """Sizes that are no multiple of any tile, anisotropic grid, off-centre
+    volume, both detector offsets, 3 channels (phantom + 2 noise fields)."""
+    kw = dict(synth.geom_kwargs(synth.CONFIGS["tiny"]))
+    kw.update(vol_nx=37, vol_ny=29, vol_nz=21, det_nu=50, det_nv=35, det_du_mm=3.0, det_dv_mm=2.7,
+              det_off_u_mm=23.0, det_off_v_mm=-4.0, vol_cx_mm=5.0, vol_cy_mm=-3.0, vol_cz_mm=2.5, n_views=11)
+    rng = np.random.default_rng(77)
+    vol = rng.random((3, 21, 29, 37), dtype=np.float32)
+    sino = rng.random((3, 11, 35, 50), dtype=np.float32)
+    check_all_three(cbct, oracle_mod, kw, vol, sino, "ragged")
+
+
+def test_noise_channels(cbct, oracle_mod):
+    """Smoothed-noise channels of config 4 (signed values, no flat regions)."""
+    kw = dict(synth.geom_kwargs(synth.CONFIGS["small_halffan"]))
+    kw.update(n_views=24)
+    vol = np.stack([synth.smoothed_noise(5, 64), synth.smoothed_noise(6, 64)])
+    og = oracle_mod.Geom(**kw)
+    r = oracle_mod.fp(og, vol.astype(np.float64))
+    g = run_fp(cbct, kw, vol)
+    assert rel_l2(g, r) <= 1e-5 and max_rel(g, r) <= 1e-4
+
+
+def test_adjoint_identity_fp32(cbct):
+    cfg = synth.CONFIGS["small_halffan"]
+    kw = synth.geom_kwargs(cfg)
+    rng = np.random.default_rng(9)
+    x = rng.random((1, 64, 64, 64), dtype=np.float32)
+    y = rng.random((1, 90, 128, 128), dtype=np.float32)
+    Ax = run_fp(cbct, kw, x)
+    Aty = run_adj(cbct, kw, y)
+    lhs, rhs = float(np.sum(Ax * y)), float(np.sum(x * Aty))
+    assert abs(lhs - rhs) / abs(lhs) <= 1e-5
+
+
+def test_slab_streaming_matches_resident(cbct, oracle_mod):
+    """A5: a work-set cap forces z-slabs; results equal the resident path
+    (forward: sum over slabs; adjoint / FDK: slab by slab) and the oracle."""
+    kw = dict(synth.geom_kwargs(synth.CONFIGS["tiny"]))
+    kw.update(vol_nz=40, n_views=12, det_off_u_mm=15.0)
+    rng = np.random.default_rng(4)
+    vol = rng.random((2, 40, 32, 32), dtype=np.float32)
+    sino = rng.random((2, 12, 48, 48), dtype=np.float32)
+    plane = 36 * 36 * 4 * 2
+    cap = 2 * (9 + 4) * plane + 16  # two buffers of 9 planes (+ padding) for 2 channels
+    g = cbct.Geometry(**kw, max_workset_bytes=cap)
+    assert g.num_slabs(2) == 5
+    og = oracle_mod.Geom(**kw)
+    for host in (False, True):
+        def put(a):
+            return torch.from_numpy(a.copy()).pin_memory() if host else dev(a)
+        out_s = torch.zeros((2,) + g.sino_shape, device="cuda")
+        g.fp(put(vol), out_s, 2)
+        torch.cuda.synchronize()
+        r = oracle_mod.fp(og, vol.astype(np.float64))
+        assert rel_l2(out_s.cpu().numpy().astype(np.float64), r) <= 1e-5
+        out_v = torch.empty((2,) + g.vol_shape).pin_memory() if host else torch.zeros((2,) + g.vol_shape, device="cuda")
+        g.bp_adjoint(dev(sino), out_v, 2)
+        torch.cuda.synchronize()
+        r = oracle_mod.bp_adjoint(og, sino.astype(np.float64))
+        assert rel_l2(out_v.cpu().numpy().astype(np.float64), r) <= 1e-4
+        g.bp_fdk(dev(sino), out_v, 2)
+        torch.cuda.synchronize()
+        r = oracle_mod.bp_fdk(og, sino.astype(np.float64))
+        assert rel_l2(out_v.cpu().numpy().astype(np.float64), r) <= 1e-5
+
+
+def test_host_buffers_numpy(cbct, oracle_mod):
+    """Pageable host buffers through the C ABI (the e2e path of bench.py)."""
+    cfg = synth.CONFIGS["tiny"]
+    kw = synth.geom_kwargs(cfg)
+    vol, sino = synth.make_volume(cfg), synth.make_sinogram(cfg)
+    g = cbct.Geometry(**kw)
+    og = oracle_mod.Geom(**kw)
+    out = np.empty((1,) + g.sino_shape, dtype=np.float32)
+    g.fp(vol, out, 1)
+    assert rel_l2(out.astype(np.float64), oracle_mod.fp(og, vol.astype(np.float64))) <= 1e-5
+    outv = np.empty((1,) + g.vol_shape, dtype=np.float32)
+    g.bp_adjoint(sino, outv, 1)
+    assert rel_l2(outv.astype(np.float64), oracle_mod.bp_adjoint(og, sino.astype(np.float64))) <= 1e-4
+    g.bp_fdk(sino, outv, 1)
+    assert rel_l2(outv.astype(np.float64), oracle_mod.bp_fdk(og, sino.astype(np.float64))) <= 1e-5
+
+
+def test_strided_views_subgeometry(cbct):
+    """R14 / PAPER.md:270: a handle with every 4th angle gives rows 0,4,8,... bit-identically."""
+    cfg = synth.CONFIGS["tiny"]
+    kw = dict(synth.geom_kwargs(cfg))
+    vol = synth.make_volume(cfg)
+    full = run_fp(cbct, kw, vol)
+    kw4 = dict(kw, n_views=9)
+    sub = run_fp(cbct, kw4, vol, angles_rad=[2 * np.pi * i / 36 for i in range(0, 36, 4)])
+    assert np.array_equal(full[:, ::4], sub)
+
+
+def test_degenerate_inputs(cbct):
+    """Zero volume / zero sinogram give exact zeros; a detector that misses the
+    volume entirely gives an exactly-zero sinogram and adjoint; outputs are overwritten."""
+    cfg = synth.CONFIGS["tiny"]
+    kw = dict(synth.geom_kwargs(cfg))
+    z = run_fp(cbct, kw, np.zeros((1, 32, 32, 32), np.float32))
+    assert np.all(z == 0.0)
+    assert np.all(run_adj(cbct, kw, np.zeros((1, 36, 48, 48), np.float32)) == 0.0)
+    assert np.all(run_fdk(cbct, kw, np.zeros((1, 36, 48, 48), np.float32)) == 0.0)
+    far = dict(kw, det_off_u_mm=900.0)
+    assert np.all(run_fp(cbct, far, synth.make_volume(cfg)) == 0.0)
+    assert np.all(run_adj(cbct, far, synth.make_sinogram(cfg)) == 0.0)
+    assert np.all(run_fdk(cbct, far, synth.make_sinogram(cfg)) == 0.0)
+    # single view, single-row detector, 1-voxel-thick volume
+    thin = dict(kw, n_views=1, det_nv=1, vol_nz=1)
+    out = run_fp(cbct, thin, np.ones((1, 1, 32, 32), np.float32))
+    assert out.shape == (1, 1, 1, 48) and np.all(np.isfinite(out)) and out.max() > 0
+
+
+def test_errors_are_loud(cbct):
+    with pytest.raises(cbct.CbctError):
+        cbct.Geometry(**dict(synth.geom_kwargs(synth.CONFIGS["tiny"]), step_vox=0.0))
+    g = cbct.Geometry(**synth.geom_kwargs(synth.CONFIGS["tiny"]))
+    with pytest.raises(cbct.CbctError):
+        g.fp(torch.zeros(5, device="cuda"), torch.zeros(g.n_sino, device="cuda"))
+    with pytest.raises(cbct.CbctError):
+        cbct.Geometry(**synth.geom_kwargs(synth.CONFIGS["tiny"]), max_workset_bytes=1000).num_slabs(1)
+
+
+@pytest.mark.parametrize("name", ["pyramid_64", "pyramid_128", "pyramid_256"])
+def test_config3_pyramid_sampled(cbct, oracle_mod, name):
+    """Config 3 at full size, in the launch configuration bench.py times:
+    2000 sampled rays, 48 sampled adjoint voxels, 2000 sampled FDK voxels, each
+    computed one by one by the oracle; plus the fp32 adjoint identity."""
+    cfg = synth.CONFIGS[name]
+    kw = synth.geom_kwargs(cfg)
+    og = oracle_mod.Geom(**kw)
+    vol, sino = synth.make_volume(cfg), synth.make_sinogram(cfg)
+    Ax = run_fp(cbct, kw, vol)
+    ridx = synth.sample_indices(11, Ax[0].size, 2000)
+    r = oracle_mod.fp_rays(og, vol.astype(np.float64), ridx)
+    gsel = Ax.reshape(1, -1)[:, ridx]
+    assert rel_l2(gsel, r) <= 1e-5, rel_l2(gsel, r)
+    floor = 1e-3 * float(np.max(np.abs(r)))
+    assert np.max(np.abs(gsel - r) / np.maximum(np.abs(r), floor)) <= 1e-4
+    Aty = run_adj(cbct, kw, sino)
+    vidx = synth.sample_indices(12, vol[0].size, 48)
+    r = oracle_mod.bp_adjoint_voxels(og, sino.astype(np.float64), vidx)
+    assert rel_l2(Aty.reshape(1, -1)[:, vidx], r) <= 1e-4
+    lhs, rhs = float(np.sum(Ax * sino)), float(np.sum(vol.astype(np.float64) * Aty))
+    assert abs(lhs - rhs) / abs(lhs) <= 1e-5, (lhs, rhs)
+    F = run_fdk(cbct, kw, sino)
+    vidx = synth.sample_indices(13, vol[0].size, 2000)
+    r = oracle_mod.bp_fdk_voxels(og, sino.astype(np.float64), vidx)
+    gsel = F.reshape(1, -1)[:, vidx]
+    assert rel_l2(gsel, r) <= 1e-5, rel_l2(gsel, r)
+    floor = 1e-3 * float(np.max(np.abs(r)))
+    assert np.max(np.abs(gsel - r) / np.maximum(np.abs(r), floor)) <= 1e-4
