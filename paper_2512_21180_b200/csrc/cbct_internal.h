@@ -34,12 +34,12 @@ struct ViewChunk {
     double2 cs[CBCT_VIEWS_PER_LAUNCH];  // (cos phi, sin phi)
 };
 
-// fp32 per-launch parameters of the FDK backprojection kernel.
+// per-launch parameters of the FDK backprojection kernel (fp64 setup, fp32 inner loop).
 struct FdkGeom {
-    float sid;              // voxel units
-    float au, bu, av, bv;   // fu_pad = au * (-X s + Y c) / U + bu ; fv_pad = av * Z / U + bv
-    float x0, y0, z0;       // centred world coordinate (voxel units) of voxel index 0
-    float fu_max, fv_max;   // clamp range upper bounds in padded pixel coordinates
+    double sid;             // voxel units
+    double au, bu, av, bv;  // fu_pad = au * (-X s + Y c) / U + bu ; fv_pad = av * Z / U + bv
+    double x0, y0, z0;      // centred world coordinate (voxel units) of voxel index 0
+    double fu_max, fv_max;  // clamp range upper bounds in padded pixel coordinates
     int nx, ny, nz;
     int zs0, zs1;           // z planes [zs0, zs1) written by this launch
     int pu, pv;             // padded sinogram pitch / rows

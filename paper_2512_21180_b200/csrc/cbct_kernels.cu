@@ -260,9 +260,13 @@ adjoint_kernel_v0(const float *__restrict__ sino, float *__restrict__ vol, const
 #define FDK_BY 4
 
 struct FdkViews {
-    float2 cs[CBCT_VIEWS_PER_LAUNCH];
+    double2 cs[CBCT_VIEWS_PER_LAUNCH];
 };
 
+// Per (x, y, view) the detector coordinates are set up in fp64 and split into
+// an integer cell and an fp32 fraction, so the fp32 work along z only ever
+// sees small magnitudes (|t| < ~32): coordinate error ~1e-6 px instead of the
+// 1.5e-5 px ulp of a raw fp32 coordinate near 256 (DESIGN.md s.6).
 __global__ void __launch_bounds__(FDK_BX *FDK_BY)
 fdk_kernel_v0(const float *__restrict__ sino, float *__restrict__ vol, const __grid_constant__ FdkGeom G,
               const __grid_constant__ FdkViews V, int view0, int accumulate, size_t vol_plane_origin)
@@ -271,32 +275,38 @@ fdk_kernel_v0(const float *__restrict__ sino, float *__restrict__ vol, const __g
     int iy = blockIdx.y * FDK_BY + threadIdx.y;
     int izb = G.zs0 + blockIdx.z * FDK_ZB;
     if (ix >= G.nx || iy >= G.ny) return;
-    float X = G.x0 + (float)ix, Y = G.y0 + (float)iy, Z0 = G.z0 + (float)izb;
+    const double X = G.x0 + (double)ix, Y = G.y0 + (double)iy, Z0 = G.z0 + (double)izb;
     float acc[FDK_ZB];
 #pragma unroll
     for (int k = 0; k < FDK_ZB; ++k) acc[k] = 0.f;
     const size_t img = (size_t)G.pu * G.pv;
     for (int i = 0; i < G.n_views; ++i) {
-        float c = V.cs[i].x, s = V.cs[i].y;
-        float U = G.sid - (X * c + Y * s);
-        float rU = 1.0f / U;
-        float fu = fmaf(G.au * (Y * c - X * s), rU, G.bu);
-        fu = fminf(fmaxf(fu, 1.0f), G.fu_max);
-        int ju;
-        float au;
-        cell_frac(fu - 0.5f, ju, au);
-        float w = G.sid * rU;
+        double c = V.cs[i].x, s = V.cs[i].y;
+        double U = G.sid - (X * c + Y * s);
+        double r = (double)__frcp_rn((float)U);
+        r = r * (2.0 - U * r);  // one Newton step: relative error ~1e-14
+        double fu = fmin(fmax(G.au * (Y * c - X * s) * r + G.bu, 1.0), G.fu_max);
+        double fuf = floor(fu);
+        int ju = (int)fuf;
+        float au = (float)(fu - fuf);
+        float w = (float)(G.sid * r);
         w *= w;
-        float dfv = G.av * rU;
+        double dfv_d = G.av * r;
+        double fv0 = Z0 * dfv_d + G.bv;
+        // keep the integer part of fv0 out of the fp32 arithmetic (clamped so the
+        // relative coordinate stays small even for voxels projecting far outside)
+        double base = floor(fmin(fmax(fv0, -64.0), G.fv_max + 64.0));
+        int jv0 = (int)base;
+        float f0 = (float)(fv0 - base), dfv = (float)dfv_d;
+        float lo = 1.0f - (float)jv0, hi = (float)(G.fv_max - base);
         const float *p = sino + (size_t)(view0 + i) * img + ju;
 #pragma unroll
         for (int k = 0; k < FDK_ZB; ++k) {
-            float fv = fmaf(Z0 + (float)k, dfv, G.bv);
-            fv = fminf(fmaxf(fv, 1.0f), G.fv_max);
-            int jv;
+            float t = fminf(fmaxf(fmaf((float)k, dfv, f0), lo), hi);
+            int jr;
             float av;
-            cell_frac(fv - 0.5f, jv, av);
-            const float *q = p + (size_t)jv * G.pu;
+            cell_frac(t - 0.5f, jr, av);
+            const float *q = p + (size_t)(jv0 + jr) * G.pu;
             float p00 = __ldg(q), p01 = __ldg(q + 1), p10 = __ldg(q + G.pu), p11 = __ldg(q + G.pu + 1);
             float b0 = fmaf(au, p01 - p00, p00), b1 = fmaf(au, p11 - p10, p10);
             acc[k] = fmaf(w, fmaf(av, b1 - b0, b0), acc[k]);
@@ -410,16 +420,16 @@ int cbct_launch_fdk(cbct_geom *g, const float *padded_sino, float *vol, int chan
     const cbct_geom_desc &d = g->d;
     double h = d.vox_mm;
     FdkGeom G;
-    G.sid = (float)(d.sid_mm / h);
-    G.au = (float)(d.sdd_mm / d.det_du_mm);  // (SDD/h) / (du/h)
-    G.av = (float)(d.sdd_mm / d.det_dv_mm);
-    G.bu = (float)(-(-0.5 * (d.det_nu - 1) * d.det_du_mm + d.det_off_u_mm) / d.det_du_mm + CBCT_PAD);
-    G.bv = (float)(-(-0.5 * (d.det_nv - 1) * d.det_dv_mm + d.det_off_v_mm) / d.det_dv_mm + CBCT_PAD);
-    G.x0 = (float)(d.vol_cx_mm / h - 0.5 * (d.vol_nx - 1));
-    G.y0 = (float)(d.vol_cy_mm / h - 0.5 * (d.vol_ny - 1));
-    G.z0 = (float)(d.vol_cz_mm / h - 0.5 * (d.vol_nz - 1));
-    G.fu_max = (float)(d.det_nu + CBCT_PAD);
-    G.fv_max = (float)(d.det_nv + CBCT_PAD);
+    G.sid = d.sid_mm / h;
+    G.au = d.sdd_mm / d.det_du_mm;  // (SDD/h) / (du/h)
+    G.av = d.sdd_mm / d.det_dv_mm;
+    G.bu = (-(-0.5 * (d.det_nu - 1) * d.det_du_mm + d.det_off_u_mm) / d.det_du_mm + CBCT_PAD);
+    G.bv = (-(-0.5 * (d.det_nv - 1) * d.det_dv_mm + d.det_off_v_mm) / d.det_dv_mm + CBCT_PAD);
+    G.x0 = d.vol_cx_mm / h - 0.5 * (d.vol_nx - 1);
+    G.y0 = d.vol_cy_mm / h - 0.5 * (d.vol_ny - 1);
+    G.z0 = d.vol_cz_mm / h - 0.5 * (d.vol_nz - 1);
+    G.fu_max = (double)(d.det_nu + CBCT_PAD);
+    G.fv_max = (double)(d.det_nv + CBCT_PAD);
     G.nx = d.vol_nx; G.ny = d.vol_ny; G.nz = d.vol_nz;
     G.zs0 = zs0; G.zs1 = zs1;
     G.pu = cbct_padded_sino_pitch(g);
@@ -432,7 +442,7 @@ int cbct_launch_fdk(cbct_geom *g, const float *padded_sino, float *vol, int chan
     for (int view0 = 0; view0 < d.n_views; view0 += CBCT_VIEWS_PER_LAUNCH) {
         int n = d.n_views - view0;
         if (n > CBCT_VIEWS_PER_LAUNCH) n = CBCT_VIEWS_PER_LAUNCH;
-        for (int i = 0; i < n; ++i) fv.cs[i] = make_float2((float)g->cosphi[view0 + i], (float)g->sinphi[view0 + i]);
+        for (int i = 0; i < n; ++i) fv.cs[i] = make_double2(g->cosphi[view0 + i], g->sinphi[view0 + i]);
         G.n_views = n;
         for (int c = 0; c < channels; ++c) {
             fdk_kernel_v0<<<grid, block, 0, st>>>(padded_sino + c * sstride, vol + c * vol_channel_stride, G, fv,
