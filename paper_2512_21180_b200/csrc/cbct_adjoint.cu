@@ -1,0 +1,318 @@
+// cbct_adjoint.cu -- A3, the matched adjoint P^T ("the Hermitian
+// adjoint" of Eq. 5; reading R8: plain transpose of the matrix cbct_fp applies):
+//     vol_c[j] = Delta * sum_{i,iv,iu,k} w(j; i,iv,iu,k) sino_c[i,iv,iu],
+//     w = prod_axis max(0, 1 - |q_axis(s_i + t_k d) - j_axis|),  t_k = (k + 1/2) Delta.
+//
+// Design (DESIGN.md s.6; evidence profiles/r1_v0.md).  The v0 kernel scattered
+// 8 RED.ADD.F32 per sample and ran at the per-SM global-atomic limit (about one
+// lane-RED per clock per SM, 370 ms per channel at 256^3 / 400 views).  v1 is an
+// exact GATHER: one thread per voxel enumerates the rays (iu, iv) whose line
+// crosses the voxel's tent support and, per ray, the lattice samples inside it:
+// the same terms as the scatter, summed in a fixed order, no atomics, no
+// zero-fill, plain coalesced stores, deterministic.
+//
+// Per (voxel, view) in the rotated frame (e1 = source direction, e2 = e_u,
+// e3 = z): the point of ray (u, v) at depth fraction lambda = t / L is
+// (sid - lambda sdd, lambda u, lambda v).  With lambda_U = U / sdd (the depth of
+// the voxel) and mu = lambda - lambda_U the offset sample - voxel is, exactly,
+//     e_x = A_x + mu N_x,  e_y = A_y + mu N_y,  e_z = a_v + mu v,
+//     a_u = lambda_U (u - u*),  a_v = lambda_U (v - v*),  (A_x, A_y) = a_u (-s, c),
+//     (N_x, N_y) = (-(c sdd + s u), -s sdd + c u),
+// all SMALL numbers (|e| < 2), so fp32 is enough after an fp64 set-up of
+// U, u*, v* per (voxel, view).  Sample k of the ray has mu_k = g (k - kU),
+// g = step / L, kU = lambda_U L / step - 1/2.
+//
+// The weights depend only on geometry, so they are shared by everything that
+// sees the same geometry: CB channels; NR voxels related by a rotation of the
+// (centred, square) grid about z -- the pair (view i, voxel j) has the weights
+// of (view i + r n/NR, voxel j rotated by r 360/NR degrees), so a thread walks
+// ALL views for its base voxel j (one quadrant of the grid) and adds
+// W(j, i) y[i + r n/NR] into the accumulator of the r-th rotated voxel -- and
+// NM = 2 voxels mirrored in z (ray iv <-> nv-1-iv).  One weight evaluation
+// then feeds NR * NM * CB accumulators.
+#include "cbct_device.cuh"
+
+struct AdjGeom {
+    double sid, sdd, inv_sdd;
+    double u0, du, inv_du, v0, dv, inv_dv;  // detector coordinate of pixel 0, pitch (voxel units)
+    double x0, y0, z0;                      // world coordinate (voxel units) of voxel index 0
+    double inv_step;
+    float step, scale;                      // ray step (voxel units); Delta in mm
+    float tz;                               // max |v| / sdd over the detector
+    int nu, nv, nx, ny, nz;
+    int bx, by;                             // base domain: ix < bx, iy < by
+    int bz0, bz1;                           // base planes [bz0, bz1)
+    int nq;                                 // views in this launch
+    int nbase;                              // n_views / NR: views i and i + nbase differ by 360/NR degrees
+};
+
+// out[c][iq][iv][iu][p] = in[c][iq + p nq][iv][iu], iq < nq = n_views / NR
+// (the NR views related by a grid rotation side by side, one vector load)
+template <int NR>
+__global__ void __launch_bounds__(256)
+interleave_views_kernel(const float *__restrict__ in, float *__restrict__ out, int nq, size_t img, int channels)
+{
+    const size_t n = (size_t)channels * nq * img;
+    for (size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x; e < n; e += (size_t)gridDim.x * blockDim.x) {
+        size_t pix = e % img, t = e / img;
+        size_t iq = t % nq, c = t / nq;
+        const float *src = in + (c * NR * nq + iq) * img + pix;
+        float vals[NR];
+#pragma unroll
+        for (int r = 0; r < NR; ++r) vals[r] = __ldg(src + (size_t)r * nq * img);
+        if (NR == 4) reinterpret_cast<float4 *>(out)[e] = make_float4(vals[0], vals[1], vals[2], vals[NR - 1]);
+        else if (NR == 2) reinterpret_cast<float2 *>(out)[e] = make_float2(vals[0], vals[NR - 1]);
+        else out[e] = vals[0];
+    }
+}
+
+template <int NR>
+__device__ __forceinline__ void load_views(const float *__restrict__ p, float (&y)[NR])
+{
+    if (NR == 4) {
+        float4 t = __ldg(reinterpret_cast<const float4 *>(p));
+        y[0] = t.x; y[1] = t.y; y[2] = t.z; y[NR - 1] = t.w;
+    } else if (NR == 2) {
+        float2 t = __ldg(reinterpret_cast<const float2 *>(p));
+        y[0] = t.x; y[NR - 1] = t.y;
+    } else {
+        y[0] = __ldg(p);
+    }
+}
+
+// y[r] <- y[(a + r) mod NR]  (a is uniform over the CTA: no divergence)
+template <int NR>
+__device__ __forceinline__ void rotate_views(float (&y)[NR], int a)
+{
+    if (NR == 2) {
+        if (a & 1) { float t = y[0]; y[0] = y[NR - 1]; y[NR - 1] = t; }
+    } else if (NR == 4) {
+        if (a & 1) { float t = y[0]; y[0] = y[1]; y[1] = y[2]; y[2] = y[NR - 1]; y[NR - 1] = t; }
+        if (a & 2) { float t = y[0]; y[0] = y[2]; y[2] = t; t = y[1]; y[1] = y[NR - 1]; y[NR - 1] = t; }
+    }
+}
+
+#define ADJ_BX 32
+#define ADJ_BY 4
+
+template <int NR, int NM, int CB>
+__global__ void __launch_bounds__(ADJ_BX *ADJ_BY)
+adjoint_gather_kernel(const float *__restrict__ sinoI, float *__restrict__ vol, const __grid_constant__ AdjGeom G,
+                      const __grid_constant__ ViewChunk V, int q0, int accumulate, size_t sino_cstride,
+                      size_t vol_cstride, int vol_z_origin)
+{
+    const int ix = blockIdx.x * ADJ_BX + threadIdx.x;
+    const int iy = blockIdx.y * ADJ_BY + threadIdx.y;
+    const int iz = G.bz0 + blockIdx.z;
+    if (ix >= G.bx || iy >= G.by) return;
+    const double X = G.x0 + ix, Y = G.y0 + iy, Z = G.z0 + iz;
+    float acc[NM][CB][NR];
+#pragma unroll
+    for (int m = 0; m < NM; ++m)
+#pragma unroll
+        for (int c = 0; c < CB; ++c)
+#pragma unroll
+            for (int r = 0; r < NR; ++r) acc[m][c][r] = 0.f;
+    const float u0f = (float)G.u0, duf = (float)G.du, v0f = (float)G.v0, dvf = (float)G.dv;
+    const float sddf = (float)G.sdd, sdd2f = (float)(G.sdd * G.sdd), inv_stepf = (float)G.inv_step;
+    const size_t img = (size_t)G.nv * G.nu;
+
+    for (int q = 0; q < G.nq; ++q) {
+        // ---- fp64 set-up of the voxel's projection (once per voxel and view) ----
+        const double c = V.cs[q].x, s = V.cs[q].y;
+        const double U = G.sid - (X * c + Y * s), w = Y * c - X * s;
+        const double rU = 1.0 / U;
+        const double ustar = G.sdd * w * rU, vstar = G.sdd * Z * rU;
+        const double fu = (ustar - G.u0) * G.inv_du, fv = (vstar - G.v0) * G.inv_dv;
+        const double lamU = U * G.inv_sdd;
+        // rays whose xy-line can cross the open square |e_x|, |e_y| < 1:
+        // |a_u| sdd < |N_x| + |N_y|  (support function of the square), N Lipschitz in u
+        const double Bu = (fabs(c * G.sdd + s * ustar) + fabs(c * ustar - s * G.sdd)) / ((U - 1.5) * G.du);
+        // rays that can have |e_z| < 1 while inside the square (|mu| sdd <= sqrt 2)
+        const double Bv = (1.0 + 1.45 * (double)G.tz) / (lamU * G.dv);
+        const int iu_lo = max(0, (int)ceil(fu - Bu)), iu_hi = min(G.nu - 1, (int)floor(fu + Bu));
+        const int iv_lo = max(0, (int)ceil(fv - Bv)), iv_hi = min(G.nv - 1, (int)floor(fv + Bv));
+        if (iu_lo > iu_hi || iv_lo > iv_hi) continue;
+        const float cf = (float)c, sf = (float)s, lamUf = (float)lamU;
+        const float lu = (float)(lamU * G.du), lv = (float)(lamU * G.dv);
+        const float dfu0 = (float)((double)iu_lo - fu), dfv0 = (float)((double)iv_lo - fv);
+        // view i = ib + a nbase: component p of the interleaved pixel is view ib + p nbase,
+        // and the r-th rotated voxel takes view i + r nbase = component (a + r) mod NR
+        const int a = (q0 + q) / G.nbase, ib = (q0 + q) - a * G.nbase;
+        const float *sq = sinoI + (size_t)ib * img * NR;
+
+        for (int iu = iu_lo; iu <= iu_hi; ++iu) {
+            const float u = fmaf((float)iu, duf, u0f);
+            const float au = lu * (dfu0 + (float)(iu - iu_lo));
+            const float Nx = -fmaf(sf, u, cf * sddf), Ny = fmaf(cf, u, -sf * sddf);
+            const float Ax = -sf * au, Ay = cf * au;
+            // window of mu from the dominant horizontal axis: |A_d + mu N_d| < 1
+            const bool domx = fabsf(Nx) >= fabsf(Ny);
+            const float invNd = __frcp_rn(domx ? Nx : Ny);
+            const float muc = -(domx ? Ax : Ay) * invNd, hw = fabsf(invNd);
+            const float lam_lo = lamUf + (muc - hw), lam_hi = lamUf + (muc + hw);
+            const float H2 = fmaf(u, u, sdd2f);
+
+            for (int iv = iv_lo; iv <= iv_hi; ++iv) {
+                const float v = fmaf((float)iv, dvf, v0f);
+                const float av = lv * (dfv0 + (float)(iv - iv_lo));
+                const float L2 = fmaf(v, v, H2);
+                float invL = rsqrtf(L2);
+                invL = fmaf(fmaf(-0.5f * L2 * invL, invL, 0.5f), invL, invL);  // one Newton step
+                if (fabsf(av) >= 1.0f + 1.45f * fabsf(v) * invL) continue;
+                const float L = L2 * invL;
+                const float invg = L * inv_stepf;  // samples per unit lambda
+                const float g = G.step * invL;     // lambda per sample
+                const float kU = fmaf(lamUf, invg, -0.5f);
+                const float klo = floorf(fmaf(lam_lo, invg, -0.5f)) + 1.0f;
+                const float khi = ceilf(fmaf(lam_hi, invg, -0.5f)) - 1.0f;
+                const float gNx = g * Nx, gNy = g * Ny, gv = g * v;
+                float W = 0.f;
+                for (float kf = klo; kf <= khi; kf += 1.0f) {
+                    const float d = kf - kU;
+                    const float wx = fmaxf(1.0f - fabsf(fmaf(d, gNx, Ax)), 0.f);
+                    const float wy = fmaxf(1.0f - fabsf(fmaf(d, gNy, Ay)), 0.f);
+                    const float wz = fmaxf(1.0f - fabsf(fmaf(d, gv, av)), 0.f);
+                    W = fmaf(wx * wy, wz, W);
+                }
+                if (W == 0.f) continue;
+                const float *p0 = sq + ((size_t)iv * G.nu + iu) * NR;
+                const float *p1 = sq + ((size_t)(G.nv - 1 - iv) * G.nu + iu) * NR;
+#pragma unroll
+                for (int cc = 0; cc < CB; ++cc) {
+                    float y[NR];
+                    load_views<NR>(p0 + cc * sino_cstride, y);
+                    rotate_views<NR>(y, a);
+#pragma unroll
+                    for (int r = 0; r < NR; ++r) acc[0][cc][r] = fmaf(W, y[r], acc[0][cc][r]);
+                    if (NM == 2) {
+                        load_views<NR>(p1 + cc * sino_cstride, y);
+                        rotate_views<NR>(y, a);
+#pragma unroll
+                        for (int r = 0; r < NR; ++r) acc[NM - 1][cc][r] = fmaf(W, y[r], acc[NM - 1][cc][r]);
+                    }
+                }
+            }
+        }
+    }
+
+    // ---- stores: rotation r maps (ix, iy) -> r quarter (NR = 4) or half (NR = 2) turns ----
+#pragma unroll
+    for (int m = 0; m < NM; ++m) {
+        const int z = m == 0 ? iz : G.nz - 1 - iz;
+        if (m == 1 && z == iz) continue;  // middle plane of an odd nz is its own mirror image
+#pragma unroll
+        for (int r = 0; r < NR; ++r) {
+            int x = ix, y = iy;
+            if (NR == 4) {
+                if (r == 1) { x = G.nx - 1 - iy; y = ix; }
+                if (r == 2) { x = G.nx - 1 - ix; y = G.ny - 1 - iy; }
+                if (r == 3) { x = iy; y = G.ny - 1 - ix; }
+            } else if (NR == 2 && r == 1) {
+                x = G.nx - 1 - ix; y = G.ny - 1 - iy;
+            }
+            const size_t o = ((size_t)(z - vol_z_origin) * G.ny + y) * G.nx + x;
+#pragma unroll
+            for (int cc = 0; cc < CB; ++cc) {
+                float val = acc[m][cc][r] * G.scale;
+                float *dst = vol + cc * vol_cstride + o;
+                *dst = accumulate ? *dst + val : val;
+            }
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------
+// launchers
+// ---------------------------------------------------------------------------
+int cbct_launch_interleave_views(cbct_geom *g, const float *sino, float *out, int channels, cudaStream_t st)
+{
+    const int NR = g->sym_rot;
+    const int nq = g->d.n_views / NR;
+    const size_t img = (size_t)g->d.det_nv * g->d.det_nu;
+    const size_t n = (size_t)channels * nq * img;
+    size_t blocks = (n + 255) / 256;
+    if (blocks > 148u * 16u) blocks = 148u * 16u;
+    if (NR == 4) interleave_views_kernel<4><<<(unsigned)blocks, 256, 0, st>>>(sino, out, nq, img, channels);
+    else if (NR == 2) interleave_views_kernel<2><<<(unsigned)blocks, 256, 0, st>>>(sino, out, nq, img, channels);
+    else return CBCT_ERR_INVALID_ARG;
+    return cbct_check_launch(g, "interleave_views_kernel");
+}
+
+template <int NR, int NM, int CB>
+static int launch_gather(cbct_geom *g, AdjGeom &G, const float *sinoI, float *vol, int accumulate_first,
+                         size_t sstride, size_t vstride, int vol_z_origin, cudaStream_t st)
+{
+    const int nq_total = g->d.n_views;
+    G.nbase = g->d.n_views / NR;
+    ViewChunk vc;
+    dim3 block(ADJ_BX, ADJ_BY);
+    dim3 grid((G.bx + ADJ_BX - 1) / ADJ_BX, (G.by + ADJ_BY - 1) / ADJ_BY, G.bz1 - G.bz0);
+    for (int q0 = 0; q0 < nq_total; q0 += CBCT_VIEWS_PER_LAUNCH) {
+        int n = nq_total - q0;
+        if (n > CBCT_VIEWS_PER_LAUNCH) n = CBCT_VIEWS_PER_LAUNCH;
+        for (int i = 0; i < n; ++i) vc.cs[i] = make_double2(g->cosphi[q0 + i], g->sinphi[q0 + i]);
+        G.nq = n;
+        adjoint_gather_kernel<NR, NM, CB><<<grid, block, 0, st>>>(sinoI, vol, G, vc, q0, accumulate_first || q0 > 0,
+                                                                  sstride, vstride, vol_z_origin);
+        int rc = cbct_check_launch(g, "adjoint_gather_kernel");
+        if (rc) return rc;
+    }
+    return CBCT_OK;
+}
+
+template <int NR, int NM>
+static int launch_gather_channels(cbct_geom *g, AdjGeom &G, const float *sinoI, float *vol, int channels,
+                                  size_t sstride, size_t vstride, int vol_z_origin, cudaStream_t st)
+{
+    int c = 0;
+    while (c < channels) {
+        int left = channels - c, rc;
+        const float *s = sinoI + c * sstride;
+        float *v = vol + c * vstride;
+        if (left >= 2 && NR * NM <= 8) { rc = launch_gather<NR, NM, 2>(g, G, s, v, 0, sstride, vstride, vol_z_origin, st); c += 2; }
+        else { rc = launch_gather<NR, NM, 1>(g, G, s, v, 0, sstride, vstride, vol_z_origin, st); c += 1; }
+        if (rc) return rc;
+    }
+    return CBCT_OK;
+}
+
+// sino_src: the sinogram as the caller laid it out if sym_rot == 1, else the
+// view-interleaved copy made by cbct_launch_interleave_views.  Writes planes
+// [zs0, zs1) of vol (whose first stored plane is vol_z_origin).  The z-mirror
+// is used only when the launch covers the whole grid.
+int cbct_launch_adjoint(cbct_geom *g, const float *sino_src, float *vol, int channels, int zs0, int zs1,
+                        size_t vol_channel_stride, int vol_z_origin, cudaStream_t st)
+{
+    const cbct_geom_desc &d = g->d;
+    const double h = d.vox_mm;
+    AdjGeom G;
+    G.sid = d.sid_mm / h; G.sdd = d.sdd_mm / h; G.inv_sdd = 1.0 / G.sdd;
+    G.du = d.det_du_mm / h; G.dv = d.det_dv_mm / h; G.inv_du = 1.0 / G.du; G.inv_dv = 1.0 / G.dv;
+    G.u0 = (-0.5 * (d.det_nu - 1) * d.det_du_mm + d.det_off_u_mm) / h;
+    G.v0 = (-0.5 * (d.det_nv - 1) * d.det_dv_mm + d.det_off_v_mm) / h;
+    G.x0 = d.vol_cx_mm / h - 0.5 * (d.vol_nx - 1);
+    G.y0 = d.vol_cy_mm / h - 0.5 * (d.vol_ny - 1);
+    G.z0 = d.vol_cz_mm / h - 0.5 * (d.vol_nz - 1);
+    G.step = (float)d.step_vox; G.inv_step = 1.0 / d.step_vox;
+    G.scale = (float)(d.step_vox * d.vox_mm);
+    double vmax = fmax(fabs(G.v0), fabs(G.v0 + (d.det_nv - 1) * G.dv));
+    G.tz = (float)(vmax / G.sdd);
+    G.nu = d.det_nu; G.nv = d.det_nv; G.nx = d.vol_nx; G.ny = d.vol_ny; G.nz = d.vol_nz;
+    const int NR = g->sym_rot;
+    const bool mirror = g->sym_mirror_z && zs0 == 0 && zs1 == d.vol_nz && d.vol_nz > 1;
+    G.bx = NR == 4 ? d.vol_nx / 2 : d.vol_nx;
+    G.by = NR >= 2 ? d.vol_ny / 2 : d.vol_ny;
+    G.bz0 = zs0; G.bz1 = mirror ? (d.vol_nz + 1) / 2 : zs1;
+    G.nq = 0;
+    const size_t sstride = (size_t)d.n_views * d.det_nv * d.det_nu;
+    if (NR == 4) {
+        return mirror ? launch_gather_channels<4, 2>(g, G, sino_src, vol, channels, sstride, vol_channel_stride, vol_z_origin, st)
+                      : launch_gather_channels<4, 1>(g, G, sino_src, vol, channels, sstride, vol_channel_stride, vol_z_origin, st);
+    } else if (NR == 2) {
+        return mirror ? launch_gather_channels<2, 2>(g, G, sino_src, vol, channels, sstride, vol_channel_stride, vol_z_origin, st)
+                      : launch_gather_channels<2, 1>(g, G, sino_src, vol, channels, sstride, vol_channel_stride, vol_z_origin, st);
+    }
+    return mirror ? launch_gather_channels<1, 2>(g, G, sino_src, vol, channels, sstride, vol_channel_stride, vol_z_origin, st)
+                  : launch_gather_channels<1, 1>(g, G, sino_src, vol, channels, sstride, vol_channel_stride, vol_z_origin, st);
+}

@@ -56,6 +56,9 @@ extern "C" int cbct_geom_create(const cbct_geom_desc *d, cbct_geom **out)
     double rc = sqrt(d->vol_cx_mm * d->vol_cx_mm + d->vol_cy_mm * d->vol_cy_mm + d->vol_cz_mm * d->vol_cz_mm);
     double rbound = rc + sqrt(hx * hx + hy * hy + hz * hz);
     if (!(rbound < d->sid_mm)) return CBCT_ERR_INVALID_ARG;
+    // ... and strictly in front of the detector plane, so every in-support
+    // sample has t_k < |p - s| (the forward sum stops at the detector).
+    if (!(rbound < d->sdd_mm - d->sid_mm)) return CBCT_ERR_INVALID_ARG;
 
     cbct_geom *g = new (std::nothrow) cbct_geom();
     if (!g) return CBCT_ERR_NOMEM;
@@ -71,6 +74,27 @@ extern "C" int cbct_geom_create(const cbct_geom_desc *d, cbct_geom **out)
         g->sinphi[i] = sin(phi);
     }
     g->d.angles_rad = g->angles.data();
+    // Symmetries the gather adjoint exploits (cbct_adjoint.cu): a centred grid and
+    // views i, i + n/R that differ by exactly 360/R degrees see the same geometry
+    // up to a rotation of the grid; a volume and detector centred in z are
+    // mirror-symmetric under z -> -z.
+    auto views_rotate = [&](int R) {
+        if (d->n_views % R) return false;
+        const int nq = d->n_views / R;
+        for (int r = 1; r < R; ++r) {
+            const double cr = cos(2.0 * M_PI * r / R), sr = sin(2.0 * M_PI * r / R);
+            for (int i = 0; i < nq; ++i) {
+                double c = g->cosphi[i] * cr - g->sinphi[i] * sr, s = g->sinphi[i] * cr + g->cosphi[i] * sr;
+                if (fabs(c - g->cosphi[i + r * nq]) > 1e-13 || fabs(s - g->sinphi[i + r * nq]) > 1e-13) return false;
+            }
+        }
+        return true;
+    };
+    const bool centred_xy = d->vol_cx_mm == 0.0 && d->vol_cy_mm == 0.0;
+    if (centred_xy && d->vol_nx == d->vol_ny && d->vol_nx % 2 == 0 && views_rotate(4)) g->sym_rot = 4;
+    else if (centred_xy && d->vol_ny % 2 == 0 && views_rotate(2)) g->sym_rot = 2;
+    else g->sym_rot = 1;
+    g->sym_mirror_z = d->vol_cz_mm == 0.0 && d->det_off_v_mm == 0.0;
     *out = g;
     return CBCT_OK;
 }
@@ -78,10 +102,11 @@ extern "C" int cbct_geom_create(const cbct_geom_desc *d, cbct_geom **out)
 extern "C" int cbct_geom_destroy(cbct_geom *g)
 {
     if (!g) return CBCT_ERR_INVALID_ARG;
-    if (g->ws_vol || g->ws_sino || g->ws_stage || g->copy_stream) {
+    if (g->ws_vol || g->ws_sino || g->ws_sino2 || g->ws_stage || g->copy_stream) {
         cudaDeviceSynchronize();
         cudaFree(g->ws_vol);
         cudaFree(g->ws_sino);
+        cudaFree(g->ws_sino2);
         cudaFree(g->ws_stage);
         for (int i = 0; i < 4; ++i)
             if (g->ev[i]) cudaEventDestroy(g->ev[i]);
@@ -115,8 +140,6 @@ RayGeom cbct_make_raygeom(const cbct_geom *g, int z0, int z1)
     r.pz = (z1 - z0) + 2 * CBCT_PAD;
     return r;
 }
-
-size_t cbct_padded_volume_elems(const RayGeom &r) { return (size_t)r.px * r.py * r.pz; }
 
 int cbct_padded_sino_pitch(const cbct_geom *g) { return (g->d.det_nu + 2 * CBCT_PAD + 3) & ~3; }
 int cbct_padded_sino_rows(const cbct_geom *g) { return g->d.det_nv + 2 * CBCT_PAD; }
@@ -169,16 +192,21 @@ extern "C" int cbct_geom_count_samples(const cbct_geom *gc, uint64_t *out)
     return CBCT_OK;
 }
 
-// z-slab plan (A5): planes per slab so that two padded slab buffers of all
-// `channels` channels fit under max_workset_bytes.  Returns planes per slab
-// (nz when everything is resident) or <= 0 if not even one plane fits.
+// z-slab plan (A5) of the forward projector: planes per slab so that two slab
+// buffers of all `channels` channels fit under max_workset_bytes.  A slab buffer
+// holds the quad-packed cells (16 B per padded cell) plus the raw planes they
+// are packed from when the caller's volume is in host memory (4 B per voxel;
+// counted always, so the plan does not depend on where the volume lives).
+// Returns planes per slab (nz when everything is resident) or <= 0 if not even
+// one plane fits.
 int cbct_plan_slab_planes(const cbct_geom *g, int channels)
 {
     RayGeom r = cbct_make_raygeom(g, 0, g->d.vol_nz);
     uint64_t cap = g->d.max_workset_bytes;
-    uint64_t plane = (uint64_t)r.px * r.py * sizeof(float) * (uint64_t)channels;
-    if (cap == 0 || plane * (uint64_t)r.pz <= cap) return g->d.vol_nz;
-    int64_t planes = (int64_t)(cap / (2 * plane)) - 2 * CBCT_PAD;
+    uint64_t packed_plane = (uint64_t)r.px * r.py * 16u * (uint64_t)channels;
+    uint64_t raw_plane = (uint64_t)r.nx * r.ny * 4u * (uint64_t)channels;
+    if (cap == 0 || packed_plane * (uint64_t)r.pz + raw_plane * (uint64_t)r.nz <= cap) return g->d.vol_nz;
+    int64_t planes = ((int64_t)(cap / 2) - (int64_t)(packed_plane * 2 * CBCT_PAD)) / (int64_t)(packed_plane + raw_plane);
     if (planes > g->d.vol_nz) planes = g->d.vol_nz;
     return (int)planes;
 }

@@ -50,13 +50,17 @@ struct cbct_geom {
     cbct_geom_desc d;
     std::vector<double> angles, cosphi, sinphi;
     // device workspace (lazily allocated, grown on demand)
-    float *ws_vol = nullptr;   size_t ws_vol_bytes = 0;    // padded volume(s)
-    float *ws_sino = nullptr;  size_t ws_sino_bytes = 0;   // padded / staged sinogram
-    float *ws_stage = nullptr; size_t ws_stage_bytes = 0;  // staging of host buffers
+    float *ws_vol = nullptr;   size_t ws_vol_bytes = 0;    // packed volume slab(s) / output staging slabs
+    float *ws_sino = nullptr;  size_t ws_sino_bytes = 0;   // device copy of a host sinogram
+    float *ws_sino2 = nullptr; size_t ws_sino2_bytes = 0;  // re-laid-out sinogram (view-interleaved / zero-bordered)
+    float *ws_stage = nullptr; size_t ws_stage_bytes = 0;  // raw planes of a host volume on their way to the pack kernel
     cudaStream_t copy_stream = nullptr;
     cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
     uint64_t launches = 0;
     int64_t sample_count = -1;
+    // symmetries of the geometry the gather adjoint may exploit (cbct_geom.cu):
+    int sym_rot = 1;        // 4 / 2 / 1: views i and i + n/sym_rot see the grid rotated by 360/sym_rot deg
+    bool sym_mirror_z = false;  // volume and detector symmetric under z -> -z
 };
 
 void cbct_set_cuda_error(cudaError_t e, const char *what);
@@ -72,25 +76,25 @@ void cbct_set_cuda_error(cudaError_t e, const char *what);
 
 // --- geometry helpers (cbct_geom.cu) ---------------------------------------
 RayGeom cbct_make_raygeom(const cbct_geom *g, int z0, int z1);
-size_t cbct_padded_volume_elems(const RayGeom &r);  // per channel
+size_t cbct_packed_volume_cells(const RayGeom &r);  // float4 cells per channel of a quad-packed slab
 int cbct_padded_sino_pitch(const cbct_geom *g);
 int cbct_padded_sino_rows(const cbct_geom *g);
 int cbct_plan_slab_planes(const cbct_geom *g, int channels);  // planes per z-slab, <1 = cap too small
 
-// --- kernel launchers (cbct_kernels.cu); all enqueue on `st` ----------------
-// pad:   src[C][nz_src][ny][nx] planes [z0,z1) -> dst[C][pz][py][px] (zero border)
-int cbct_launch_pad_volume(cbct_geom *g, const RayGeom &r, const float *src, float *dst, int channels,
-                           size_t src_channel_stride, int src_z_origin, cudaStream_t st);
-// unpad: padded dst planes -> vol[C][..] planes [z0,z1)
-int cbct_launch_unpad_volume(cbct_geom *g, const RayGeom &r, const float *padded, float *dst, int channels,
-                             size_t dst_channel_stride, int dst_z_origin, cudaStream_t st);
-int cbct_launch_pad_sino(cbct_geom *g, const float *src, float *dst, int channels, cudaStream_t st);
-// forward projection of the padded volume(s); accumulate != 0 adds into sino
-int cbct_launch_fp(cbct_geom *g, const RayGeom &r, const float *padded, float *sino, int channels,
+// --- kernel launchers; all enqueue on `st` ----------------------------------
+int cbct_check_launch(cbct_geom *g, const char *what);
+// quad-pack: src[C][nz_src][ny][nx] planes [r.z0, r.z1) -> dst[C][pz][py][px] float4 cells (cbct_fp.cu)
+int cbct_launch_pack_volume(cbct_geom *g, const RayGeom &r, const float *src, float4 *dst, int channels,
+                            size_t src_channel_stride, int src_z_origin, cudaStream_t st);
+// forward projection of the packed slab(s); accumulate != 0 adds into sino
+int cbct_launch_fp(cbct_geom *g, const RayGeom &r, const float4 *packed, float *sino, int channels,
                    int accumulate, cudaStream_t st);
-// adjoint scatter into zeroed padded volume(s)
-int cbct_launch_adjoint(cbct_geom *g, const RayGeom &r, const float *sino, float *padded, int channels,
-                        cudaStream_t st);
+// view-interleaved copy of the sinogram for the gather adjoint (only if g->sym_rot > 1)
+int cbct_launch_interleave_views(cbct_geom *g, const float *sino, float *out, int channels, cudaStream_t st);
+// gather adjoint into vol planes [zs0, zs1)
+int cbct_launch_adjoint(cbct_geom *g, const float *sino_src, float *vol, int channels, int zs0, int zs1,
+                        size_t vol_channel_stride, int vol_z_origin, cudaStream_t st);
+int cbct_launch_pad_sino(cbct_geom *g, const float *src, float *dst, int channels, cudaStream_t st);
 // FDK backprojection from the padded sinogram into vol planes [zs0, zs1)
 int cbct_launch_fdk(cbct_geom *g, const float *padded_sino, float *vol, int channels, int zs0, int zs1,
                     size_t vol_channel_stride, int vol_z_origin, cudaStream_t st);
