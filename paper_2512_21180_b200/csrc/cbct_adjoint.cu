@@ -80,6 +80,20 @@ __device__ __forceinline__ void load_views(const float *__restrict__ p, float (&
     }
 }
 
+__device__ __forceinline__ float rcp_approx(float x)
+{
+    float r;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+    return r;
+}
+
+__device__ __forceinline__ float rsqrt_approx(float x)
+{
+    float r;
+    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+    return r;
+}
+
 // y[r] <- y[(a + r) mod NR]  (a is uniform over the CTA: no divergence)
 template <int NR>
 __device__ __forceinline__ void rotate_views(float (&y)[NR], int a)
@@ -115,6 +129,7 @@ adjoint_gather_kernel(const float *__restrict__ sinoI, float *__restrict__ vol, 
             for (int r = 0; r < NR; ++r) acc[m][c][r] = 0.f;
     const float u0f = (float)G.u0, duf = (float)G.du, v0f = (float)G.v0, dvf = (float)G.dv;
     const float sddf = (float)G.sdd, sdd2f = (float)(G.sdd * G.sdd), inv_stepf = (float)G.inv_step;
+    const float zcull = 1.4143f * (float)G.inv_sdd;
     const size_t img = (size_t)G.nv * G.nu;
 
     for (int q = 0; q < G.nq; ++q) {
@@ -140,6 +155,15 @@ adjoint_gather_kernel(const float *__restrict__ sinoI, float *__restrict__ vol, 
         // and the r-th rotated voxel takes view i + r nbase = component (a + r) mod NR
         const int a = (q0 + q) / G.nbase, ib = (q0 + q) - a * G.nbase;
         const float *sq = sinoI + (size_t)ib * img * NR;
+        // this view's sums, by stored component (added into acc, rotated by a, after the view:
+        // two-level summation keeps the fp32 error at sqrt(#views) ulp, not sqrt(#terms) ulp)
+        float accv[NM][CB][NR];
+#pragma unroll
+        for (int m = 0; m < NM; ++m)
+#pragma unroll
+            for (int cc = 0; cc < CB; ++cc)
+#pragma unroll
+                for (int r = 0; r < NR; ++r) accv[m][cc][r] = 0.f;
 
         for (int iu = iu_lo; iu <= iu_hi; ++iu) {
             const float u = fmaf((float)iu, duf, u0f);
@@ -148,52 +172,61 @@ adjoint_gather_kernel(const float *__restrict__ sinoI, float *__restrict__ vol, 
             const float Ax = -sf * au, Ay = cf * au;
             // window of mu from the dominant horizontal axis: |A_d + mu N_d| < 1
             const bool domx = fabsf(Nx) >= fabsf(Ny);
-            const float invNd = __frcp_rn(domx ? Nx : Ny);
+            const float invNd = rcp_approx(domx ? Nx : Ny);
             const float muc = -(domx ? Ax : Ay) * invNd, hw = fabsf(invNd);
             const float lam_lo = lamUf + (muc - hw), lam_hi = lamUf + (muc + hw);
             const float H2 = fmaf(u, u, sdd2f);
+            int i0 = (iv_lo * G.nu + iu) * NR, i1 = ((G.nv - 1 - iv_lo) * G.nu + iu) * NR;
+            float v = fmaf((float)iv_lo, dvf, v0f), av = lv * dfv0;
 
-            for (int iv = iv_lo; iv <= iv_hi; ++iv) {
-                const float v = fmaf((float)iv, dvf, v0f);
-                const float av = lv * (dfv0 + (float)(iv - iv_lo));
+            for (int iv = iv_lo; iv <= iv_hi; ++iv, i0 += G.nu * NR, i1 -= G.nu * NR, v += dvf, av += lv) {
                 const float L2 = fmaf(v, v, H2);
-                float invL = rsqrtf(L2);
+                float invL = rsqrt_approx(L2);
                 invL = fmaf(fmaf(-0.5f * L2 * invL, invL, 0.5f), invL, invL);  // one Newton step
-                if (fabsf(av) >= 1.0f + 1.45f * fabsf(v) * invL) continue;
+                // inside the square |mu| sdd <= sqrt 2, so |e_z - a_v| = |mu v| <= sqrt 2 |v| / sdd
+                if (fabsf(av) >= fmaf(fabsf(v), zcull, 1.0f)) continue;
                 const float L = L2 * invL;
                 const float invg = L * inv_stepf;  // samples per unit lambda
                 const float g = G.step * invL;     // lambda per sample
-                const float kU = fmaf(lamUf, invg, -0.5f);
-                const float klo = floorf(fmaf(lam_lo, invg, -0.5f)) + 1.0f;
-                const float khi = ceilf(fmaf(lam_hi, invg, -0.5f)) - 1.0f;
+                // first sample with (k + 1/2) g > lam_lo: k = rn(lam_lo invg); a tie (weight 0) may go either way
+                const float klo = (fmaf(lam_lo, invg, CBCT_MAGIC)) - CBCT_MAGIC;
                 const float gNx = g * Nx, gNy = g * Ny, gv = g * v;
+                const float d0 = klo - fmaf(lamUf, invg, -0.5f);  // k - kU
+                float ex = fmaf(d0, gNx, Ax), ey = fmaf(d0, gNy, Ay), ez = fmaf(d0, gv, av);
                 float W = 0.f;
-                for (float kf = klo; kf <= khi; kf += 1.0f) {
-                    const float d = kf - kU;
-                    const float wx = fmaxf(1.0f - fabsf(fmaf(d, gNx, Ax)), 0.f);
-                    const float wy = fmaxf(1.0f - fabsf(fmaf(d, gNy, Ay)), 0.f);
-                    const float wz = fmaxf(1.0f - fabsf(fmaf(d, gv, av)), 0.f);
+                // the window holds at most 4 sqrt 2 < 6 samples; samples past it have weight 0 (clamps)
+#pragma unroll
+                for (int j = 0; j < 6; ++j) {
+                    const float wx = fmaxf(1.0f - fabsf(ex), 0.f);
+                    const float wy = fmaxf(1.0f - fabsf(ey), 0.f);
+                    const float wz = fmaxf(1.0f - fabsf(ez), 0.f);
                     W = fmaf(wx * wy, wz, W);
+                    if (j == 3 && fmaf(lam_hi, invg, -4.5f) <= klo) break;  // k = klo + 4 is past the window
+                    ex += gNx; ey += gNy; ez += gv;
                 }
                 if (W == 0.f) continue;
-                const float *p0 = sq + ((size_t)iv * G.nu + iu) * NR;
-                const float *p1 = sq + ((size_t)(G.nv - 1 - iv) * G.nu + iu) * NR;
 #pragma unroll
                 for (int cc = 0; cc < CB; ++cc) {
                     float y[NR];
-                    load_views<NR>(p0 + cc * sino_cstride, y);
-                    rotate_views<NR>(y, a);
+                    load_views<NR>(sq + cc * sino_cstride + i0, y);
 #pragma unroll
-                    for (int r = 0; r < NR; ++r) acc[0][cc][r] = fmaf(W, y[r], acc[0][cc][r]);
+                    for (int r = 0; r < NR; ++r) accv[0][cc][r] = fmaf(W, y[r], accv[0][cc][r]);
                     if (NM == 2) {
-                        load_views<NR>(p1 + cc * sino_cstride, y);
-                        rotate_views<NR>(y, a);
+                        load_views<NR>(sq + cc * sino_cstride + i1, y);
 #pragma unroll
-                        for (int r = 0; r < NR; ++r) acc[NM - 1][cc][r] = fmaf(W, y[r], acc[NM - 1][cc][r]);
+                        for (int r = 0; r < NR; ++r) accv[NM - 1][cc][r] = fmaf(W, y[r], accv[NM - 1][cc][r]);
                     }
                 }
             }
         }
+#pragma unroll
+        for (int m = 0; m < NM; ++m)
+#pragma unroll
+            for (int cc = 0; cc < CB; ++cc) {
+                rotate_views<NR>(accv[m][cc], a);
+#pragma unroll
+                for (int r = 0; r < NR; ++r) acc[m][cc][r] += accv[m][cc][r];
+            }
     }
 
     // ---- stores: rotation r maps (ix, iy) -> r quarter (NR = 4) or half (NR = 2) turns ----

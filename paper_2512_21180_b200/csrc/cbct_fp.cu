@@ -12,7 +12,18 @@
 // LDG.32.  The packed buffer carries a zero border of CBCT_PAD cells, which
 // implements the zero-extension boundary rule R4 with no bounds test in the
 // loop.  CB channels share the position / weight arithmetic of a sample.
+#include <stdlib.h>
+
 #include "cbct_device.cuh"
+
+// Position of cell jx inside its row: the cell keeps its 128-byte line (8 cells) but
+// rotates inside it by a (jy, jz)-dependent amount, so that neighbouring rows and
+// planes put the same jx on different L1 data banks (a quarter-warp's LDG.128 reads
+// ~5 distinct cells of a 2-D patch; un-swizzled, equal jx in different rows collide).
+__device__ __forceinline__ int cbct_swizzle(int jx, int jy, int jz, int swy, int swz)
+{
+    return (jx & ~7) | ((jx + swy * jy + swz * jz) & 7);
+}
 
 // ---------------------------------------------------------------------------
 // quad-pack pass: src[C][nz_src][ny][nx] planes [z0, z1) -> packed[C][pz][py][px] float4
@@ -44,7 +55,7 @@ pack_volume_kernel(const float *__restrict__ src, float4 *__restrict__ dst, cons
                 if (okx1) q.w = __ldg(r + x1);
             }
         }
-        d[(size_t)row * G.px + jx] = q;
+        d[(size_t)row * G.px + cbct_swizzle(jx, jy, jz, G.swy, G.swz)] = q;
     }
 }
 
@@ -56,12 +67,23 @@ pack_volume_kernel(const float *__restrict__ src, float4 *__restrict__ dst, cons
 
 __device__ __forceinline__ float lerpf(float a, float b, float t) { return fmaf(t, b - a, a); }
 
-__device__ __forceinline__ float quad_sample(const float4 *__restrict__ p, int plane, float fx, float fy, float fz)
+__device__ __forceinline__ float quad_sample(const float4 *__restrict__ p0, const float4 *__restrict__ p1, float fx,
+                                             float fy, float fz)
 {
-    float4 q0 = __ldg(p), q1 = __ldg(p + plane);
+    float4 q0 = __ldg(p0), q1 = __ldg(p1);
     float b0 = lerpf(lerpf(q0.x, q0.y, fx), lerpf(q0.z, q0.w, fx), fy);
     float b1 = lerpf(lerpf(q1.x, q1.y, fx), lerpf(q1.z, q1.w, fx), fy);
     return lerpf(b0, b1, fz);
+}
+
+// Addresses of the cells (jx, jy, jz) and (jx, jy, jz + 1) of the packed slab.
+__device__ __forceinline__ void cell_pointers(const float4 *__restrict__ packed, const RayGeom &G, int jx, int jy, int jz,
+                                              const float4 *&p0, const float4 *&p1)
+{
+    const int row = (jz * G.py + jy) * G.px + (jx & ~7);
+    const int t = jx + G.swy * jy + G.swz * jz;
+    p0 = packed + (row + (t & 7));
+    p1 = packed + (row + G.px * G.py + ((t + G.swz) & 7));
 }
 
 // CB channels per thread; a warp covers TU x (32 / TU) pixels; CTA = 16 x 16 pixels.
@@ -78,7 +100,6 @@ fp_kernel(const float4 *__restrict__ packed, float *__restrict__ sino, const __g
     if (iu >= G.nu || iv >= G.nv) return;
     const int view = blockIdx.z;
     const Ray r = cbct_ray_setup(G, V.cs[view].x, V.cs[view].y, iu, iv);
-    const int rowp = G.px, plane = G.px * G.py;
     float acc[CB], acc2[CB];
 #pragma unroll
     for (int c = 0; c < CB; ++c) acc[c] = acc2[c] = 0.f;
@@ -94,12 +115,13 @@ fp_kernel(const float4 *__restrict__ packed, float *__restrict__ sino, const __g
         cbct_cell_frac(fmaf(kg, r.dx, r.ax), kx, gx);
         cbct_cell_frac(fmaf(kg, r.dy, r.ay), ky, gy);
         cbct_cell_frac(fmaf(kg, r.dz, r.az), kz, gz);
-        const float4 *p = packed + ((jz * G.py + jy) * rowp + jx);
-        const float4 *q = packed + ((kz * G.py + ky) * rowp + kx);
+        const float4 *p0, *p1, *q0, *q1;
+        cell_pointers(packed, G, jx, jy, jz, p0, p1);
+        cell_pointers(packed, G, kx, ky, kz, q0, q1);
 #pragma unroll
         for (int c = 0; c < CB; ++c) {
-            acc[c] += quad_sample(p + c * packed_cstride, plane, fx, fy, fz);
-            acc2[c] += quad_sample(q + c * packed_cstride, plane, gx, gy, gz);
+            acc[c] += quad_sample(p0 + c * packed_cstride, p1 + c * packed_cstride, fx, fy, fz);
+            acc2[c] += quad_sample(q0 + c * packed_cstride, q1 + c * packed_cstride, gx, gy, gz);
         }
     }
     if (it < r.n) {
@@ -108,9 +130,11 @@ fp_kernel(const float4 *__restrict__ packed, float *__restrict__ sino, const __g
         cbct_cell_frac(fmaf(kf, r.dx, r.ax), jx, fx);
         cbct_cell_frac(fmaf(kf, r.dy, r.ay), jy, fy);
         cbct_cell_frac(fmaf(kf, r.dz, r.az), jz, fz);
-        const float4 *p = packed + ((jz * G.py + jy) * rowp + jx);
+        const float4 *p0, *p1;
+        cell_pointers(packed, G, jx, jy, jz, p0, p1);
 #pragma unroll
-        for (int c = 0; c < CB; ++c) acc[c] += quad_sample(p + c * packed_cstride, plane, fx, fy, fz);
+        for (int c = 0; c < CB; ++c)
+            acc[c] += quad_sample(p0 + c * packed_cstride, p1 + c * packed_cstride, fx, fy, fz);
     }
     const float delta = (float)G.delta;
     const size_t o = ((size_t)(view0 + view) * G.nv + iv) * G.nu + iu;
@@ -143,7 +167,10 @@ static int launch_fp_cb(cbct_geom *g, const RayGeom &r, const ViewChunk &vc, int
                         cudaStream_t st)
 {
     dim3 grid((r.nu + FP_CTA_U - 1) / FP_CTA_U, (r.nv + FP_CTA_V - 1) / FP_CTA_V, nviews);
-    fp_kernel<CB, 8><<<grid, FP_CTA_U * FP_CTA_V, 0, st>>>(packed, sino, r, vc, view0, accumulate, pstride, sstride);
+    static const int tu = getenv("CBCT_FP_TU") ? atoi(getenv("CBCT_FP_TU")) : 8;  // TODO(tuning): remove
+    if (tu == 4) fp_kernel<CB, 4><<<grid, FP_CTA_U * FP_CTA_V, 0, st>>>(packed, sino, r, vc, view0, accumulate, pstride, sstride);
+    else if (tu == 16) fp_kernel<CB, 16><<<grid, FP_CTA_U * FP_CTA_V, 0, st>>>(packed, sino, r, vc, view0, accumulate, pstride, sstride);
+    else fp_kernel<CB, 8><<<grid, FP_CTA_U * FP_CTA_V, 0, st>>>(packed, sino, r, vc, view0, accumulate, pstride, sstride);
     return cbct_check_launch(g, "fp_kernel");
 }
 
@@ -152,6 +179,7 @@ int cbct_launch_fp(cbct_geom *g, const RayGeom &r, const float4 *packed, float *
 {
     const size_t pstride = cbct_packed_volume_cells(r);
     const size_t sstride = (size_t)g->d.n_views * r.nv * r.nu;
+    static const int cbmax = getenv("CBCT_FP_CB") ? atoi(getenv("CBCT_FP_CB")) : 4;  // TODO(tuning): remove
     ViewChunk vc;  // 8 KB; copied into the launch's parameter buffer at launch time
     for (int view0 = 0; view0 < g->d.n_views; view0 += CBCT_VIEWS_PER_LAUNCH) {
         int n = g->d.n_views - view0;
@@ -162,8 +190,8 @@ int cbct_launch_fp(cbct_geom *g, const RayGeom &r, const float4 *packed, float *
             int left = channels - c, rc;
             const float4 *p = packed + c * pstride;
             float *s = sino + c * sstride;
-            if (left >= 4) { rc = launch_fp_cb<4>(g, r, vc, n, view0, p, s, accumulate, pstride, sstride, st); c += 4; }
-            else if (left >= 2) { rc = launch_fp_cb<2>(g, r, vc, n, view0, p, s, accumulate, pstride, sstride, st); c += 2; }
+            if (left >= 4 && cbmax >= 4) { rc = launch_fp_cb<4>(g, r, vc, n, view0, p, s, accumulate, pstride, sstride, st); c += 4; }
+            else if (left >= 2 && cbmax >= 2) { rc = launch_fp_cb<2>(g, r, vc, n, view0, p, s, accumulate, pstride, sstride, st); c += 2; }
             else { rc = launch_fp_cb<1>(g, r, vc, n, view0, p, s, accumulate, pstride, sstride, st); c += 1; }
             if (rc) return rc;
         }

@@ -169,7 +169,7 @@ def test_slab_streaming_matches_resident(cbct, oracle_mod):
     rng = np.random.default_rng(4)
     vol = rng.random((2, 40, 32, 32), dtype=np.float32)
     sino = rng.random((2, 12, 48, 48), dtype=np.float32)
-    packed, raw = 36 * 36 * 16 * 2, 32 * 32 * 4 * 2   # bytes per plane, 2 channels (quad-packed cells, raw voxels)
+    packed, raw = 40 * 36 * 16 * 2, 32 * 32 * 4 * 2   # bytes per plane, 2 channels (quad-packed cells, raw voxels)
     cap = 2 * (9 * (packed + raw) + 4 * packed) + 16   # two slab buffers of 9 planes (+ 4 border planes)
     g = cbct.Geometry(**kw, max_workset_bytes=cap)
     assert g.num_slabs(2) == 5
