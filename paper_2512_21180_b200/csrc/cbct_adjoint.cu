@@ -66,46 +66,6 @@ interleave_views_kernel(const float *__restrict__ in, float *__restrict__ out, i
     }
 }
 
-template <int NR>
-__device__ __forceinline__ void load_views(const float *__restrict__ p, float (&y)[NR])
-{
-    if (NR == 4) {
-        float4 t = __ldg(reinterpret_cast<const float4 *>(p));
-        y[0] = t.x; y[1] = t.y; y[2] = t.z; y[NR - 1] = t.w;
-    } else if (NR == 2) {
-        float2 t = __ldg(reinterpret_cast<const float2 *>(p));
-        y[0] = t.x; y[NR - 1] = t.y;
-    } else {
-        y[0] = __ldg(p);
-    }
-}
-
-__device__ __forceinline__ float rcp_approx(float x)
-{
-    float r;
-    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
-    return r;
-}
-
-__device__ __forceinline__ float rsqrt_approx(float x)
-{
-    float r;
-    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
-    return r;
-}
-
-// y[r] <- y[(a + r) mod NR]  (a is uniform over the CTA: no divergence)
-template <int NR>
-__device__ __forceinline__ void rotate_views(float (&y)[NR], int a)
-{
-    if (NR == 2) {
-        if (a & 1) { float t = y[0]; y[0] = y[NR - 1]; y[NR - 1] = t; }
-    } else if (NR == 4) {
-        if (a & 1) { float t = y[0]; y[0] = y[1]; y[1] = y[2]; y[2] = y[NR - 1]; y[NR - 1] = t; }
-        if (a & 2) { float t = y[0]; y[0] = y[2]; y[2] = t; t = y[1]; y[1] = y[NR - 1]; y[NR - 1] = t; }
-    }
-}
-
 #define ADJ_BX 32
 #define ADJ_BY 4
 

@@ -248,24 +248,21 @@ extern "C" int cbct_bp_fdk(const cbct_geom *gc, const float *sino, float *vol, i
     cbct_geom *g = cx.g;
     cudaStream_t st = cx.st;
 
+    // zero-bordered, rotation-interleaved copy of the sinogram (cbct_fdk.cu)
     const int pu = cbct_padded_sino_pitch(g), pv = cbct_padded_sino_rows(g);
     const size_t psino = (size_t)g->d.n_views * pu * pv * channels;
+    const size_t sino_bytes = cx.nsino * channels * sizeof(float);
+    const float *d_sino = sino;
+    if (cx.ks != MEM_DEVICE) {
+        rc = ensure(&g->ws_sino, &g->ws_sino_bytes, sino_bytes);
+        if (rc) return rc;
+        CBCT_CUDA_TRY(cudaMemcpyAsync(g->ws_sino, sino, sino_bytes, cudaMemcpyHostToDevice, st));
+        d_sino = g->ws_sino;
+    }
     rc = ensure(&g->ws_sino2, &g->ws_sino2_bytes, psino * sizeof(float));
     if (rc) return rc;
-    if (cx.ks == MEM_DEVICE) {
-        rc = cbct_launch_pad_sino(g, sino, g->ws_sino2, channels, st);
-        if (rc) return rc;
-    } else {  // one pitched copy straight into the interior of the zeroed padded buffer
-        CBCT_CUDA_TRY(cudaMemsetAsync(g->ws_sino2, 0, psino * sizeof(float), st));
-        cudaMemcpy3DParms p;
-        memset(&p, 0, sizeof(p));
-        p.srcPtr = make_cudaPitchedPtr((void *)sino, g->d.det_nu * sizeof(float), g->d.det_nu, g->d.det_nv);
-        p.dstPtr = make_cudaPitchedPtr((void *)g->ws_sino2, pu * sizeof(float), pu, pv);
-        p.dstPos = make_cudaPos(CBCT_PAD * sizeof(float), CBCT_PAD, 0);
-        p.extent = make_cudaExtent(g->d.det_nu * sizeof(float), g->d.det_nv, (size_t)g->d.n_views * channels);
-        p.kind = cudaMemcpyHostToDevice;
-        CBCT_CUDA_TRY(cudaMemcpy3DAsync(&p, st));
-    }
+    rc = cbct_launch_pad_sino(g, d_sino, g->ws_sino2, channels, st);
+    if (rc) return rc;
     const float *padded = g->ws_sino2;
     rc = produce_volume(cx, vol, [&](float *dst, int zs0, int zs1, size_t cstride, int z_origin) {
         return cbct_launch_fdk(g, padded, dst, channels, zs0, zs1, cstride, z_origin, st);

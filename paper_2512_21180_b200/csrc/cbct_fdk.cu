@@ -1,6 +1,18 @@
 // cbct_fdk.cu -- A4, the voxel-driven FDK-weighted backprojection (PAPER.md:157,
 // :181 Alg. 1 l.3, ref [9] :397; readings R9-R11 in DESIGN.md s.3):
-//     vol_c[z,y,x] = sum_i (SID/U_i)^2 * B[sino_c,i](fv, fu).
+//     vol_c[z,y,x] = sum_i (SID/U_i)^2 * B[sino_c,i](fv, fu),
+//     U_i = SID - (x cos phi_i + y sin phi_i),  u* = SDD (-x sin phi_i + y cos phi_i) / U_i,
+//     v* = SDD z / U_i,  B = zero-extended bilinear interpolation on the detector.
+//
+// Design (DESIGN.md s.6).  One thread per (x, y) column with ZB consecutive z in
+// registers: per (x, y, view) one fp64 set-up (U, 1/U, u*, weight); along z, u*
+// and the weight are constant and v* is affine.  As in the gather adjoint the
+// geometry of (view i, voxel j) equals that of (view i + r n/NR, voxel j rotated
+// by r 360/NR degrees) and of the z-mirrored voxel with detector row nv-1-iv, so
+// a thread owns a base column in one quadrant / the lower half and accumulates
+// NR * NM voxels from one coordinate computation.  The sinogram is re-laid out
+// once per call with a zero border (no bounds tests; boundary rule R10) and with
+// the NR rotation-related views side by side (one LDG.128 per tap for 4 views).
 #include "cbct_device.cuh"
 
 int cbct_check_launch(cbct_geom *g, const char *what)
@@ -11,36 +23,37 @@ int cbct_check_launch(cbct_geom *g, const char *what)
     return CBCT_OK;
 }
 
-static unsigned grid_for(size_t n, int block)
+// out[c][ib][pv][pu][p] = in[c][ib + p nb][v][u] inside the detector, 0 on the border
+template <int NR>
+__global__ void __launch_bounds__(256)
+pad_sino_kernel(const float *__restrict__ in, float *__restrict__ out, int nu, int nv, int pu, int pv, int nb,
+                int channels)
 {
-    size_t b = (n + block - 1) / block;
-    size_t cap = 148u * 32u;
-    return (unsigned)(b < cap ? (b ? b : 1) : cap);
-}
-
-// zero-bordered copy of the sinogram: rows = channels * views * pv padded rows
-__global__ void pad_sino_kernel(const float *__restrict__ src, float *__restrict__ dst, int nu, int nv, int pu,
-                                int pv, size_t n_rows_total)
-{
-    // rows = channels * views * pv padded rows
-    size_t n = n_rows_total * pu;
+    const size_t pimg = (size_t)pu * pv, img = (size_t)nu * nv;
+    const size_t n = (size_t)channels * nb * pimg;
     for (size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x; e < n; e += (size_t)gridDim.x * blockDim.x) {
-        int u = (int)(e % pu) - CBCT_PAD;
-        size_t row = e / pu;
-        int v = (int)(row % pv) - CBCT_PAD;
-        size_t img = row / pv;
-        float val = 0.f;
-        if (u >= 0 && u < nu && v >= 0 && v < nv) val = src[(img * nv + v) * nu + u];
-        dst[e] = val;
+        const int u = (int)(e % pu) - CBCT_PAD;
+        size_t t = e / pu;
+        const int v = (int)(t % pv) - CBCT_PAD;
+        t /= pv;
+        const size_t ib = t % nb, c = t / nb;
+        float vals[NR];
+#pragma unroll
+        for (int r = 0; r < NR; ++r) vals[r] = 0.f;
+        if (u >= 0 && u < nu && v >= 0 && v < nv) {
+            const float *src = in + (c * NR * nb + ib) * img + (size_t)v * nu + u;
+#pragma unroll
+            for (int r = 0; r < NR; ++r) vals[r] = __ldg(src + (size_t)r * nb * img);
+        }
+        if (NR == 4) reinterpret_cast<float4 *>(out)[e] = make_float4(vals[0], vals[1], vals[2], vals[NR - 1]);
+        else if (NR == 2) reinterpret_cast<float2 *>(out)[e] = make_float2(vals[0], vals[NR - 1]);
+        else out[e] = vals[0];
     }
 }
 
 // ---------------------------------------------------------------------------
-// A4 FDK backprojection, v0: thread per (x, y) with FDK_ZB consecutive z in
-// registers; per (x, y, view): one reciprocal, u* and the weight are constant
-// along z and v* is affine in z.  Taps come from the zero-padded sinogram.
+// backprojection kernel
 // ---------------------------------------------------------------------------
-#define FDK_ZB 8
 #define FDK_BX 32
 #define FDK_BY 4
 
@@ -52,59 +65,117 @@ struct FdkViews {
 // an integer cell and an fp32 fraction, so the fp32 work along z only ever
 // sees small magnitudes (|t| < ~32): coordinate error ~1e-6 px instead of the
 // 1.5e-5 px ulp of a raw fp32 coordinate near 256 (DESIGN.md s.6).
+template <int NR, int NM, int ZB>
 __global__ void __launch_bounds__(FDK_BX *FDK_BY)
-fdk_kernel_v0(const float *__restrict__ sino, float *__restrict__ vol, const __grid_constant__ FdkGeom G,
-              const __grid_constant__ FdkViews V, int view0, int accumulate, size_t vol_plane_origin)
+fdk_kernel(const float *__restrict__ sinoP, float *__restrict__ vol, const __grid_constant__ FdkGeom G,
+           const __grid_constant__ FdkViews V, int q0, int accumulate, int vol_z_origin)
 {
-    int ix = blockIdx.x * FDK_BX + threadIdx.x;
-    int iy = blockIdx.y * FDK_BY + threadIdx.y;
-    int izb = G.zs0 + blockIdx.z * FDK_ZB;
-    if (ix >= G.nx || iy >= G.ny) return;
+    const int ix = blockIdx.x * FDK_BX + threadIdx.x;
+    const int iy = blockIdx.y * FDK_BY + threadIdx.y;
+    const int izb = G.bz0 + blockIdx.z * ZB;
+    if (ix >= G.bx || iy >= G.by) return;
     const double X = G.x0 + (double)ix, Y = G.y0 + (double)iy, Z0 = G.z0 + (double)izb;
-    float acc[FDK_ZB];
+    float acc[NM][ZB][NR];
 #pragma unroll
-    for (int k = 0; k < FDK_ZB; ++k) acc[k] = 0.f;
-    const size_t img = (size_t)G.pu * G.pv;
-    for (int i = 0; i < G.n_views; ++i) {
-        double c = V.cs[i].x, s = V.cs[i].y;
-        double U = G.sid - (X * c + Y * s);
+    for (int m = 0; m < NM; ++m)
+#pragma unroll
+        for (int k = 0; k < ZB; ++k)
+#pragma unroll
+            for (int r = 0; r < NR; ++r) acc[m][k][r] = 0.f;
+    const size_t pimg = (size_t)G.pu * G.pv;
+    const int rowstride = G.pu * NR;
+    int a_prev = q0 / G.nbase;
+
+    for (int q = 0; q < G.n_views; ++q) {
+        // during the views of block a the accumulator of the r-th rotated voxel is
+        // component (r + a) mod NR, matching the stored component of view i + r nbase
+        const int a = (q0 + q) / G.nbase, ib = (q0 + q) - a * G.nbase;
+        if (NR > 1 && a != a_prev) {
+#pragma unroll
+            for (int m = 0; m < NM; ++m)
+#pragma unroll
+                for (int k = 0; k < ZB; ++k) rotate_views<NR>(acc[m][k], NR - (a - a_prev));
+            a_prev = a;
+        }
+        const double c = V.cs[q].x, s = V.cs[q].y;
+        const double U = G.sid - (X * c + Y * s);
         double r = (double)__frcp_rn((float)U);
         r = r * (2.0 - U * r);  // one Newton step: relative error ~1e-14
-        double fu = fmin(fmax(G.au * (Y * c - X * s) * r + G.bu, 1.0), G.fu_max);
-        double fuf = floor(fu);
-        int ju = (int)fuf;
-        float au = (float)(fu - fuf);
+        const double fu = fmin(fmax(G.au * (Y * c - X * s) * r + G.bu, 1.0), G.fu_max);
+        const double fuf = floor(fu);
+        const int ju = (int)fuf;
+        const float au = (float)(fu - fuf);
         float w = (float)(G.sid * r);
         w *= w;
-        double dfv_d = G.av * r;
-        double fv0 = Z0 * dfv_d + G.bv;
+        const double dfv_d = G.av * r;
+        const double fv0 = Z0 * dfv_d + G.bv;
         // keep the integer part of fv0 out of the fp32 arithmetic (clamped so the
         // relative coordinate stays small even for voxels projecting far outside)
-        double base = floor(fmin(fmax(fv0, -64.0), G.fv_max + 64.0));
-        int jv0 = (int)base;
-        float f0 = (float)(fv0 - base), dfv = (float)dfv_d;
-        float lo = 1.0f - (float)jv0, hi = (float)(G.fv_max - base);
-        const float *p = sino + (size_t)(view0 + i) * img + ju;
+        const double base = floor(fmin(fmax(fv0, -64.0), G.fv_max + 64.0));
+        const int jv0 = (int)base;
+        const float f0 = (float)(fv0 - base), dfv = (float)dfv_d;
+        const float lo = 1.0f - (float)jv0, hi = (float)(G.fv_max - base);
+        const float *p = sinoP + ((size_t)ib * pimg + ju) * NR;
 #pragma unroll
-        for (int k = 0; k < FDK_ZB; ++k) {
-            float t = fminf(fmaxf(fmaf((float)k, dfv, f0), lo), hi);
+        for (int k = 0; k < ZB; ++k) {
+            const float t = fminf(fmaxf(fmaf((float)k, dfv, f0), lo), hi);
             int jr;
             float av;
             cbct_cell_frac(t - 0.5f, jr, av);
-            const float *q = p + (size_t)(jv0 + jr) * G.pu;
-            float p00 = __ldg(q), p01 = __ldg(q + 1), p10 = __ldg(q + G.pu), p11 = __ldg(q + G.pu + 1);
-            float b0 = fmaf(au, p01 - p00, p00), b1 = fmaf(au, p11 - p10, p10);
-            acc[k] = fmaf(w, fmaf(av, b1 - b0, b0), acc[k]);
-        }
-    }
+            const int row = jv0 + jr;
+            {
+                const float *q00 = p + row * rowstride;
+                float y00[NR], y01[NR], y10[NR], y11[NR];
+                load_views<NR>(q00, y00);
+                load_views<NR>(q00 + NR, y01);
+                load_views<NR>(q00 + rowstride, y10);
+                load_views<NR>(q00 + rowstride + NR, y11);
 #pragma unroll
-    for (int k = 0; k < FDK_ZB; ++k) {
-        int iz = izb + k;
-        if (iz < G.zs1) {
-            size_t o = ((size_t)iz * G.ny + iy) * G.nx + ix - vol_plane_origin;
-            vol[o] = accumulate ? vol[o] + acc[k] : acc[k];
+                for (int rr = 0; rr < NR; ++rr) {
+                    const float b0 = fmaf(au, y01[rr] - y00[rr], y00[rr]), b1 = fmaf(au, y11[rr] - y10[rr], y10[rr]);
+                    acc[0][k][rr] = fmaf(w, fmaf(av, b1 - b0, b0), acc[0][k][rr]);
+                }
+            }
+            if (NM == 2) {  // voxel mirrored in z: rows pv-2-row and pv-1-row, fraction 1 - av
+                const float *q00 = p + (G.pv - 2 - row) * rowstride;
+                float y00[NR], y01[NR], y10[NR], y11[NR];
+                load_views<NR>(q00, y00);
+                load_views<NR>(q00 + NR, y01);
+                load_views<NR>(q00 + rowstride, y10);
+                load_views<NR>(q00 + rowstride + NR, y11);
+#pragma unroll
+                for (int rr = 0; rr < NR; ++rr) {
+                    const float b0 = fmaf(au, y01[rr] - y00[rr], y00[rr]), b1 = fmaf(au, y11[rr] - y10[rr], y10[rr]);
+                    acc[NM - 1][k][rr] = fmaf(w, fmaf(av, b0 - b1, b1), acc[NM - 1][k][rr]);
+                }
+            }
         }
     }
+
+    // ---- stores ----
+#pragma unroll
+    for (int m = 0; m < NM; ++m)
+#pragma unroll
+        for (int k = 0; k < ZB; ++k) {
+            const int izk = izb + k;
+            if (izk >= G.bz1) continue;
+            const int z = m == 0 ? izk : G.nz - 1 - izk;
+            if (m == 1 && z == izk) continue;  // middle plane of an odd nz is its own mirror image
+            rotate_views<NR>(acc[m][k], a_prev);
+#pragma unroll
+            for (int r = 0; r < NR; ++r) {
+                int x = ix, y = iy;
+                if (NR == 4) {
+                    if (r == 1) { x = G.nx - 1 - iy; y = ix; }
+                    if (r == 2) { x = G.nx - 1 - ix; y = G.ny - 1 - iy; }
+                    if (r == 3) { x = iy; y = G.ny - 1 - ix; }
+                } else if (NR == 2 && r == 1) {
+                    x = G.nx - 1 - ix; y = G.ny - 1 - iy;
+                }
+                float *dst = vol + ((size_t)(z - vol_z_origin) * G.ny + y) * G.nx + x;
+                *dst = accumulate ? *dst + acc[m][k][r] : acc[m][k][r];
+            }
+        }
 }
 
 // ---------------------------------------------------------------------------
@@ -112,17 +183,50 @@ fdk_kernel_v0(const float *__restrict__ sino, float *__restrict__ vol, const __g
 // ---------------------------------------------------------------------------
 int cbct_launch_pad_sino(cbct_geom *g, const float *src, float *dst, int channels, cudaStream_t st)
 {
-    int pu = cbct_padded_sino_pitch(g), pv = cbct_padded_sino_rows(g);
-    size_t rows = (size_t)channels * g->d.n_views * pv;
-    pad_sino_kernel<<<grid_for(rows * pu, 256), 256, 0, st>>>(src, dst, g->d.det_nu, g->d.det_nv, pu, pv, rows);
+    const int NR = g->sym_rot, nb = g->d.n_views / NR;
+    const int pu = cbct_padded_sino_pitch(g), pv = cbct_padded_sino_rows(g);
+    const size_t n = (size_t)channels * nb * pu * pv;
+    size_t blocks = (n + 255) / 256;
+    if (blocks > 148u * 16u) blocks = 148u * 16u;
+    if (NR == 4) pad_sino_kernel<4><<<(unsigned)blocks, 256, 0, st>>>(src, dst, g->d.det_nu, g->d.det_nv, pu, pv, nb, channels);
+    else if (NR == 2) pad_sino_kernel<2><<<(unsigned)blocks, 256, 0, st>>>(src, dst, g->d.det_nu, g->d.det_nv, pu, pv, nb, channels);
+    else pad_sino_kernel<1><<<(unsigned)blocks, 256, 0, st>>>(src, dst, g->d.det_nu, g->d.det_nv, pu, pv, nb, channels);
     return cbct_check_launch(g, "pad_sino_kernel");
 }
 
+template <int NR, int NM, int ZB>
+static int launch_fdk(cbct_geom *g, FdkGeom &G, const float *padded, float *vol, int channels, size_t vstride,
+                      int vol_z_origin, cudaStream_t st)
+{
+    const cbct_geom_desc &d = g->d;
+    const size_t sstride = (size_t)d.n_views * G.pu * G.pv;  // floats per channel of the re-laid-out sinogram
+    G.nbase = d.n_views / NR;
+    FdkViews fv;
+    dim3 block(FDK_BX, FDK_BY);
+    dim3 grid((G.bx + FDK_BX - 1) / FDK_BX, (G.by + FDK_BY - 1) / FDK_BY, (G.bz1 - G.bz0 + ZB - 1) / ZB);
+    for (int q0 = 0; q0 < d.n_views; q0 += CBCT_VIEWS_PER_LAUNCH) {
+        int n = d.n_views - q0;
+        if (n > CBCT_VIEWS_PER_LAUNCH) n = CBCT_VIEWS_PER_LAUNCH;
+        for (int i = 0; i < n; ++i) fv.cs[i] = make_double2(g->cosphi[q0 + i], g->sinphi[q0 + i]);
+        G.n_views = n;
+        for (int c = 0; c < channels; ++c) {
+            fdk_kernel<NR, NM, ZB><<<grid, block, 0, st>>>(padded + c * sstride, vol + c * vstride, G, fv, q0, q0 > 0,
+                                                           vol_z_origin);
+            int rc = cbct_check_launch(g, "fdk_kernel");
+            if (rc) return rc;
+        }
+    }
+    return CBCT_OK;
+}
+
+// `padded_sino` is the output of cbct_launch_pad_sino.  Writes planes [zs0, zs1) of vol
+// (whose first stored plane is vol_z_origin); the z-mirror is used only when the
+// launch covers the whole grid.
 int cbct_launch_fdk(cbct_geom *g, const float *padded_sino, float *vol, int channels, int zs0, int zs1,
                     size_t vol_channel_stride, int vol_z_origin, cudaStream_t st)
 {
     const cbct_geom_desc &d = g->d;
-    double h = d.vox_mm;
+    const double h = d.vox_mm;
     FdkGeom G;
     G.sid = d.sid_mm / h;
     G.au = d.sdd_mm / d.det_du_mm;  // (SDD/h) / (du/h)
@@ -135,25 +239,19 @@ int cbct_launch_fdk(cbct_geom *g, const float *padded_sino, float *vol, int chan
     G.fu_max = (double)(d.det_nu + CBCT_PAD);
     G.fv_max = (double)(d.det_nv + CBCT_PAD);
     G.nx = d.vol_nx; G.ny = d.vol_ny; G.nz = d.vol_nz;
-    G.zs0 = zs0; G.zs1 = zs1;
     G.pu = cbct_padded_sino_pitch(g);
     G.pv = cbct_padded_sino_rows(g);
-    size_t sstride = (size_t)d.n_views * G.pu * G.pv;
-    size_t origin = (size_t)vol_z_origin * d.vol_ny * d.vol_nx;
-    FdkViews fv;
-    dim3 block(FDK_BX, FDK_BY);
-    dim3 grid((d.vol_nx + FDK_BX - 1) / FDK_BX, (d.vol_ny + FDK_BY - 1) / FDK_BY, (zs1 - zs0 + FDK_ZB - 1) / FDK_ZB);
-    for (int view0 = 0; view0 < d.n_views; view0 += CBCT_VIEWS_PER_LAUNCH) {
-        int n = d.n_views - view0;
-        if (n > CBCT_VIEWS_PER_LAUNCH) n = CBCT_VIEWS_PER_LAUNCH;
-        for (int i = 0; i < n; ++i) fv.cs[i] = make_double2(g->cosphi[view0 + i], g->sinphi[view0 + i]);
-        G.n_views = n;
-        for (int c = 0; c < channels; ++c) {
-            fdk_kernel_v0<<<grid, block, 0, st>>>(padded_sino + c * sstride, vol + c * vol_channel_stride, G, fv,
-                                                  view0, view0 > 0, origin);
-            int rc = cbct_check_launch(g, "fdk_kernel_v0");
-            if (rc) return rc;
-        }
-    }
-    return CBCT_OK;
+    const int NR = g->sym_rot;
+    const bool mirror = g->sym_mirror_z && zs0 == 0 && zs1 == d.vol_nz && d.vol_nz > 1;
+    G.bx = NR == 4 ? d.vol_nx / 2 : d.vol_nx;
+    G.by = NR >= 2 ? d.vol_ny / 2 : d.vol_ny;
+    G.bz0 = zs0; G.bz1 = mirror ? (d.vol_nz + 1) / 2 : zs1;
+    G.n_views = 0; G.nbase = 0;
+    const size_t vs = vol_channel_stride;
+    if (NR == 4) return mirror ? launch_fdk<4, 2, 4>(g, G, padded_sino, vol, channels, vs, vol_z_origin, st)
+                               : launch_fdk<4, 1, 8>(g, G, padded_sino, vol, channels, vs, vol_z_origin, st);
+    if (NR == 2) return mirror ? launch_fdk<2, 2, 8>(g, G, padded_sino, vol, channels, vs, vol_z_origin, st)
+                               : launch_fdk<2, 1, 8>(g, G, padded_sino, vol, channels, vs, vol_z_origin, st);
+    return mirror ? launch_fdk<1, 2, 8>(g, G, padded_sino, vol, channels, vs, vol_z_origin, st)
+                  : launch_fdk<1, 1, 8>(g, G, padded_sino, vol, channels, vs, vol_z_origin, st);
 }

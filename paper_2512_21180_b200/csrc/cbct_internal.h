@@ -45,9 +45,11 @@ struct FdkGeom {
     double x0, y0, z0;      // centred world coordinate (voxel units) of voxel index 0
     double fu_max, fv_max;  // clamp range upper bounds in padded pixel coordinates
     int nx, ny, nz;
-    int zs0, zs1;           // z planes [zs0, zs1) written by this launch
+    int bx, by;             // base columns: ix < bx, iy < by (a quadrant / half if views rotate)
+    int bz0, bz1;           // base planes [bz0, bz1) (the lower half if the z-mirror is used)
     int pu, pv;             // padded sinogram pitch / rows
-    int n_views;
+    int n_views;            // views in this launch
+    int nbase;              // n_views_total / sym_rot
 };
 
 struct cbct_geom {

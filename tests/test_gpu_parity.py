@@ -128,10 +128,10 @@ def test_noise_channels(cbct, oracle_mod):
     dict(n_views=8, vol_ny=31, vol_nx=31),             # odd grid: no rotation
     dict(n_views=8, irregular=True),                   # non-equispaced angles: no rotation
 ])
-def test_adjoint_symmetry_paths(cbct, oracle_mod, case):
-    """The gather adjoint shares weights between views related by a grid rotation and
+def test_backprojector_symmetry_paths(cbct, oracle_mod, case):
+    """Both backprojectors share geometry between views related by a grid rotation and
     between z-mirrored voxels when the geometry allows; every combination must equal
-    the oracle's plain transpose, 3 channels (odd count: both channel-block sizes)."""
+    the oracle (adjoint: its plain transpose), 3 channels (odd count: both channel-block sizes)."""
     case = dict(case)
     kw = dict(synth.geom_kwargs(synth.CONFIGS["tiny"]))
     irregular = case.pop("irregular", False)
@@ -147,6 +147,10 @@ def test_adjoint_symmetry_paths(cbct, oracle_mod, case):
     g = run_adj(cbct, kw, sino, **extra)
     assert rel_l2(g, r) <= 1e-4, rel_l2(g, r)
     assert max_rel(g, r) <= 1e-3, max_rel(g, r)
+    r = oracle_mod.bp_fdk(og, sino.astype(np.float64))
+    g = run_fdk(cbct, kw, sino, **extra)
+    assert rel_l2(g, r) <= 1e-5, rel_l2(g, r)
+    assert max_rel(g, r) <= 1e-4, max_rel(g, r)
 
 
 def test_adjoint_identity_fp32(cbct):
