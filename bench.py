@@ -27,6 +27,11 @@ METRIC = "forward Gsamples/s at 256^3 (backprojection Gvoxel-views/s in `backpro
 UNIT = "Gsamples/s"
 
 
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of each kernel at the default workload,
+# from the ncu --set full capture summarised in profiles/ (None = not captured for this build).
+NCU_DRAM_BYTES_PER_LAUNCH = {"fp_kernel": None, "adjoint_gather_kernel": None, "fdk_kernel": None}
+
+
 def peaks():
     try:
         with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
@@ -103,8 +108,7 @@ def oracle_sample(cfg, steps, warmup):
 
 
 def run_reference(args, cfg):
-    rank = int(os.environ.get("RANK", "0"))
-    if rank != 0:
+    if int(os.environ.get("RANK", "0")) != 0:
         return
     cb, dt = oracle_sample(cfg, max(1, min(args.steps, 3)), min(args.warmup, 1))
     line = {"impl": "reference", "metric": METRIC, "value": cb["value"], "unit": UNIT, "n_gpus": args.gpus,
@@ -140,10 +144,9 @@ def main():
     import torch
     import torch.distributed as dist
     from paper_2512_21180_b200 import cbct
+    from paper_2512_21180_b200 import dist as cdist
 
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
+    rank, local, world = cdist.env_world()
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback")
     torch.cuda.set_device(local)
@@ -176,36 +179,31 @@ def main():
         if ev:
             ev[3].record()
 
-    def barrier():
-        torch.cuda.synchronize()
-        if world > 1:
-            dist.barrier()
-        torch.cuda.synchronize()
-
     for _ in range(args.warmup):
         step()
-    barrier()
+    cdist.barrier(cuda=True)
     l0 = g.launch_count()
+    g.profile(True)   # CUDA-event pair around every fp / adjoint / fdk kernel launch, on their stream
     evs = [[torch.cuda.Event(enable_timing=True) for _ in range(4)] for _ in range(args.steps)]
     with ClockSampler(local) as clk:
         for k in range(args.steps):
             step(evs[k])
-        barrier()
+        cdist.barrier(cuda=True)
+    g.profile(False)
     launches = g.launch_count() - l0
+    kern = {name: g.profile_read(i) for i, name in enumerate(("fp_kernel", "adjoint_gather_kernel", "fdk_kernel"))}
     t_fp = sum(e[0].elapsed_time(e[1]) for e in evs) / args.steps
     t_adj = sum(e[1].elapsed_time(e[2]) for e in evs) / args.steps
     t_fdk = sum(e[2].elapsed_time(e[3]) for e in evs) / args.steps
     t_total = evs[0][0].elapsed_time(evs[-1][3]) / args.steps
-    tt = torch.tensor([t_fp, t_adj, t_fdk, t_total], device="cuda", dtype=torch.float64)
-    if world > 1:
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-    t_fp, t_adj, t_fdk, t_total = [float(x) for x in tt.cpu()]
+    t_fp, t_adj, t_fdk, t_total = cdist.max_over_ranks([t_fp, t_adj, t_fdk, t_total], device="cuda")
 
     # end to end through the C ABI with HOST (pinned) buffers: copies inside the timed region
     e2e = None
     if not args.no_e2e:
         hv, hs = torch.from_numpy(vol_h).pin_memory(), torch.from_numpy(sino_h).pin_memory()
         hso, hvo = torch.empty_like(hs).pin_memory(), torch.empty_like(hv).pin_memory()
+
         def e2e_step(ev=None):
             if ev:
                 ev[0].record()
@@ -217,16 +215,13 @@ def main():
             if ev:
                 ev[2].record()
         e2e_step()
-        barrier()
+        cdist.barrier(cuda=True)
         ev2 = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(args.steps)]
         for k in range(args.steps):
             e2e_step(ev2[k])
-        barrier()
-        te = torch.tensor([sum(e[0].elapsed_time(e[1]) for e in ev2) / args.steps,
-                           ev2[0][0].elapsed_time(ev2[-1][2]) / args.steps], device="cuda", dtype=torch.float64)
-        if world > 1:
-            dist.all_reduce(te, op=dist.ReduceOp.MAX)
-        te_fp, te_step = [float(x) for x in te.cpu()]
+        cdist.barrier(cuda=True)
+        te_fp, te_step = cdist.max_over_ranks([sum(e[0].elapsed_time(e[1]) for e in ev2) / args.steps,
+                                               ev2[0][0].elapsed_time(ev2[-1][2]) / args.steps], device="cuda")
         e2e = {"value": world * C * n_samples / (te_fp * 1e-3) / 1e9, "unit": UNIT,
                "h2d_bytes_per_step": int(vol_h.nbytes + 2 * sino_h.nbytes),
                "d2h_bytes_per_step": int(sino_h.nbytes + 2 * vol_h.nbytes),
@@ -244,29 +239,42 @@ def main():
     fwd = world * C * n_samples / (t_fp * 1e-3) / 1e9
     adj_vv = world * C * n_vv / (t_adj * 1e-3) / 1e9
     fdk_vv = world * C * n_vv / (t_fdk * 1e-3) / 1e9
-    # roofline of the dominant call (see DESIGN.md s.7): algorithmic on-SM tap bytes
-    # per unit (fp 32 B/sample, adjoint 64 B/sample, fdk 16 B/voxel-view) against
-    # 148 SMs x 128 B/clk at the SM clock seen under load.
+    # Roofline of the dominant kernel (DESIGN.md s.7).  Algorithmic on-SM bytes per unit:
+    # forward 32 B per sample (8 taps x 4 B through L1), adjoint 64 B per sample (the scatter form's
+    # 8 tap read-modify-writes; the gather does less), FDK 16 B per voxel-view; peak =
+    # 148 SMs x 128 B/clk x the SM clock sampled during the timed region.  Launch durations are the
+    # library's own CUDA-event pairs around each kernel launch, on the launching stream.
     l1_peak = 148 * 128 * sm_hz / 1e9
-    calls = {"cbct_fp": (t_fp, 32.0 * C * n_samples), "cbct_bp_adjoint": (t_adj, 64.0 * C * n_samples),
-             "cbct_bp_fdk": (t_fdk, 16.0 * C * n_vv)}
-    dom = max(calls, key=lambda k: calls[k][0])
-    ach = calls[dom][1] / (calls[dom][0] * 1e-3) / 1e9
-    hbm_bytes = {"cbct_fp": C * 4.0 * (g.n_vol + g.n_sino), "cbct_bp_adjoint": C * 4.0 * (g.n_vol + g.n_sino),
-                 "cbct_bp_fdk": C * 4.0 * (g.n_vol + g.n_sino)}
-    roofline = {"kernel": dom, "bound": "l1", "achieved": ach, "peak": l1_peak, "unit": "GB/s",
-                "frac": ach / l1_peak, "traffic": None,
-                "peak_source": f"148 SM x 128 B/clk x {sm_hz / 1e6:.0f} MHz (on-SM L1/shared pipe; "
-                               "HBM is not the bound: see hbm_frac)",
-                "hbm_frac": hbm_bytes[dom] / (calls[dom][0] * 1e-3) / 1e9 / pk["hbm_gbs"],
-                "hbm_peak_source": pk_src,
-                "per_call": {k: {"ms": v[0], "l1_frac": v[1] / (v[0] * 1e-3) / 1e9 / l1_peak} for k, v in calls.items()}}
+    work = {"fp_kernel": 32.0 * C * n_samples, "adjoint_gather_kernel": 64.0 * C * n_samples,
+            "fdk_kernel": 16.0 * C * n_vv}     # algorithmic bytes per step
+    per_kernel = {}
+    for name, (ms, n) in kern.items():
+        if n == 0:
+            continue
+        avg = ms / n
+        per_launch = work[name] * args.steps / n
+        per_kernel[name] = {"launches": n, "avg_launch_ms": avg, "achieved_gbs": per_launch / (avg * 1e-3) / 1e9,
+                            "frac": per_launch / (avg * 1e-3) / 1e9 / l1_peak,
+                            "share_of_step": ms / args.steps / t_total}
+    dom = max(per_kernel, key=lambda k: kern[k][0])
+    hbm_alg = C * 4.0 * (g.n_vol + g.n_sino) * args.steps / kern[dom][1]
+    roofline = {"kernel": dom, "bound": "l1", "achieved": per_kernel[dom]["achieved_gbs"], "peak": l1_peak,
+                "unit": "GB/s", "frac": per_kernel[dom]["frac"], "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get(dom),
+                "peak_source": f"derived: 148 SM x 128 B/clk x {sm_hz / 1e6:.0f} MHz (L1 data path; MEASURED_PEAKS.json "
+                               "has no L1 figure; HBM is not the bound, see hbm_frac)",
+                "traffic_source": "profiles/r1_final.md (ncu --set full, dram__bytes_read.sum + dram__bytes_write.sum)",
+                "hbm_frac": hbm_alg / (per_kernel[dom]["avg_launch_ms"] * 1e-3) / 1e9 / pk["hbm_gbs"],
+                "hbm_peak_gbs": pk["hbm_gbs"], "hbm_peak_source": pk_src,
+                "per_kernel": per_kernel,
+                "note": "adjoint frac is against the scatter-form 64 B/sample figure; the gather shares weights "
+                        "across rotated views / mirrored voxels / channels and can read above 1"}
     line = {"metric": METRIC, "value": fwd, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": t_total, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f32", "data": "synthetic",
             "config": {"workload": cfg["name"], "volume": [cfg["vol_nz"], cfg["vol_ny"], cfg["vol_nx"]],
                        "vox_mm": cfg["vox_mm"], "views": cfg["n_views"], "detector": [cfg["det_nv"], cfg["det_nu"]],
                        "channels": C, "step_vox": cfg["step_vox"], "l2": "inputs larger than L2 (no flush)",
+                       "step": "cbct_fp + cbct_bp_adjoint + cbct_bp_fdk over all channels",
                        "sharding": "each rank runs its own C-channel batch; no data-path collective"},
             "backprojection": {"adjoint_gvoxel_views_per_s": adj_vv, "adjoint_gsamples_per_s":
                                world * C * n_samples / (t_adj * 1e-3) / 1e9,

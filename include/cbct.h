@@ -127,6 +127,17 @@ int cbct_geom_num_slabs(const cbct_geom *g, int32_t channels, int32_t *out);
 /* Kernels launched by this handle since creation (for bench.py's gpu_launches). */
 int cbct_geom_launch_count(const cbct_geom *g, uint64_t *out);
 
+/* Per-kernel device timing for roofline reports.  cbct_geom_profile(g, 1) clears the
+ * records and makes every later launch of the three main kernels record a CUDA-event
+ * pair on the stream it is launched on; cbct_geom_profile(g, 0) stops recording.
+ * cbct_geom_profile_read waits for the recorded events and returns, for `kernel`
+ * (CBCT_KERNEL_FP / _ADJOINT / _FDK), the summed launch durations in ms and the launch count. */
+#define CBCT_KERNEL_FP 0
+#define CBCT_KERNEL_ADJOINT 1
+#define CBCT_KERNEL_FDK 2
+int cbct_geom_profile(cbct_geom *g, int enable);
+int cbct_geom_profile_read(cbct_geom *g, int kernel, double *ms_total, uint64_t *launches);
+
 /* Static description of a status code. */
 const char *cbct_status_string(int status);
 

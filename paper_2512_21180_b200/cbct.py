@@ -20,6 +20,7 @@ LIB_PATH = os.path.join(_HERE, "libcbct.so")
 EXPORTS = (
     "cbct_geom_create", "cbct_geom_destroy", "cbct_fp", "cbct_bp_adjoint", "cbct_bp_fdk",
     "cbct_geom_count_samples", "cbct_geom_num_slabs", "cbct_geom_launch_count",
+    "cbct_geom_profile", "cbct_geom_profile_read",
     "cbct_status_string", "cbct_last_cuda_error",
 )
 
@@ -66,6 +67,9 @@ def load_library() -> ctypes.CDLL:
     L.cbct_geom_count_samples.argtypes = [vp, ctypes.POINTER(ctypes.c_uint64)]
     L.cbct_geom_num_slabs.argtypes = [vp, i32, ctypes.POINTER(i32)]
     L.cbct_geom_launch_count.argtypes = [vp, ctypes.POINTER(ctypes.c_uint64)]
+    L.cbct_geom_profile.argtypes = [vp, ctypes.c_int]
+    L.cbct_geom_profile_read.argtypes = [vp, ctypes.c_int, ctypes.POINTER(ctypes.c_double),
+                                         ctypes.POINTER(ctypes.c_uint64)]
     L.cbct_status_string.argtypes = [ctypes.c_int]
     L.cbct_status_string.restype = ctypes.c_char_p
     L.cbct_last_cuda_error.restype = ctypes.c_char_p
@@ -178,6 +182,16 @@ class Geometry:
         out = ctypes.c_int32()
         _check(load_library().cbct_geom_num_slabs(self._h, channels, ctypes.byref(out)))
         return int(out.value)
+
+    def profile(self, enable: bool = True):
+        """cbct_geom_profile: record a CUDA-event pair around every main-kernel launch."""
+        _check(load_library().cbct_geom_profile(self._h, 1 if enable else 0))
+
+    def profile_read(self, kernel: int):
+        """cbct_geom_profile_read: (summed launch ms, launches) of kernel 0 fp / 1 adjoint / 2 fdk."""
+        ms, n = ctypes.c_double(), ctypes.c_uint64()
+        _check(load_library().cbct_geom_profile_read(self._h, kernel, ctypes.byref(ms), ctypes.byref(n)))
+        return float(ms.value), int(n.value)
 
     def launch_count(self) -> int:
         out = ctypes.c_uint64()

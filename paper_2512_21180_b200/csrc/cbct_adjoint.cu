@@ -246,8 +246,10 @@ static int launch_gather(cbct_geom *g, AdjGeom &G, const float *sinoI, float *vo
         if (n > CBCT_VIEWS_PER_LAUNCH) n = CBCT_VIEWS_PER_LAUNCH;
         for (int i = 0; i < n; ++i) vc.cs[i] = make_double2(g->cosphi[q0 + i], g->sinphi[q0 + i]);
         G.nq = n;
+        cbct_prof_begin(g, CBCT_KERNEL_ADJOINT, st);
         adjoint_gather_kernel<NR, NM, CB><<<grid, block, 0, st>>>(sinoI, vol, G, vc, q0, accumulate_first || q0 > 0,
                                                                   sstride, vstride, vol_z_origin);
+        cbct_prof_end(g, CBCT_KERNEL_ADJOINT, st);
         int rc = cbct_check_launch(g, "adjoint_gather_kernel");
         if (rc) return rc;
     }

@@ -210,8 +210,10 @@ static int launch_fdk(cbct_geom *g, FdkGeom &G, const float *padded, float *vol,
         for (int i = 0; i < n; ++i) fv.cs[i] = make_double2(g->cosphi[q0 + i], g->sinphi[q0 + i]);
         G.n_views = n;
         for (int c = 0; c < channels; ++c) {
+            cbct_prof_begin(g, CBCT_KERNEL_FDK, st);
             fdk_kernel<NR, NM, ZB><<<grid, block, 0, st>>>(padded + c * sstride, vol + c * vstride, G, fv, q0, q0 > 0,
                                                            vol_z_origin);
+            cbct_prof_end(g, CBCT_KERNEL_FDK, st);
             int rc = cbct_check_launch(g, "fdk_kernel");
             if (rc) return rc;
         }

@@ -96,9 +96,11 @@ fp_kernel(const float4 *__restrict__ packed, float *__restrict__ sino, const __g
     constexpr int TV = 32 / TU, WU = FP_CTA_U / TU;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int iu = blockIdx.x * FP_CTA_U + (warp % WU) * TU + (lane % TU);
-    const int iv = blockIdx.y * FP_CTA_V + (warp / WU) * TV + (lane / TU);
+    // grid = (u tiles, views, v bands): CTAs in flight share a band of detector rows, i.e. a thin
+    // z-slab of the volume, which then stays L2-resident across all views
+    const int iv = blockIdx.z * FP_CTA_V + (warp / WU) * TV + (lane / TU);
     if (iu >= G.nu || iv >= G.nv) return;
-    const int view = blockIdx.z;
+    const int view = blockIdx.y;
     const Ray r = cbct_ray_setup(G, V.cs[view].x, V.cs[view].y, iu, iv);
     float acc[CB], acc2[CB];
 #pragma unroll
@@ -146,6 +148,7 @@ fp_kernel(const float4 *__restrict__ packed, float *__restrict__ sino, const __g
     }
 }
 
+
 // ---------------------------------------------------------------------------
 // launchers
 // ---------------------------------------------------------------------------
@@ -166,11 +169,13 @@ static int launch_fp_cb(cbct_geom *g, const RayGeom &r, const ViewChunk &vc, int
                         const float4 *packed, float *sino, int accumulate, size_t pstride, size_t sstride,
                         cudaStream_t st)
 {
-    dim3 grid((r.nu + FP_CTA_U - 1) / FP_CTA_U, (r.nv + FP_CTA_V - 1) / FP_CTA_V, nviews);
+    dim3 grid((r.nu + FP_CTA_U - 1) / FP_CTA_U, nviews, (r.nv + FP_CTA_V - 1) / FP_CTA_V);
+    cbct_prof_begin(g, CBCT_KERNEL_FP, st);
     static const int tu = getenv("CBCT_FP_TU") ? atoi(getenv("CBCT_FP_TU")) : 8;  // TODO(tuning): remove
     if (tu == 4) fp_kernel<CB, 4><<<grid, FP_CTA_U * FP_CTA_V, 0, st>>>(packed, sino, r, vc, view0, accumulate, pstride, sstride);
     else if (tu == 16) fp_kernel<CB, 16><<<grid, FP_CTA_U * FP_CTA_V, 0, st>>>(packed, sino, r, vc, view0, accumulate, pstride, sstride);
     else fp_kernel<CB, 8><<<grid, FP_CTA_U * FP_CTA_V, 0, st>>>(packed, sino, r, vc, view0, accumulate, pstride, sstride);
+    cbct_prof_end(g, CBCT_KERNEL_FP, st);
     return cbct_check_launch(g, "fp_kernel");
 }
 

@@ -100,6 +100,8 @@ extern "C" int cbct_geom_create(const cbct_geom_desc *d, cbct_geom **out)
     return CBCT_OK;
 }
 
+static void prof_clear(cbct_geom *g);
+
 extern "C" int cbct_geom_destroy(cbct_geom *g)
 {
     if (!g) return CBCT_ERR_INVALID_ARG;
@@ -111,6 +113,7 @@ extern "C" int cbct_geom_destroy(cbct_geom *g)
         cudaFree(g->ws_stage);
         for (int i = 0; i < 4; ++i)
             if (g->ev[i]) cudaEventDestroy(g->ev[i]);
+        prof_clear(g);
         if (g->copy_stream) cudaStreamDestroy(g->copy_stream);
     }
     delete g;
@@ -220,6 +223,52 @@ extern "C" int cbct_geom_num_slabs(const cbct_geom *g, int32_t channels, int32_t
     int planes = cbct_plan_slab_planes(g, channels);
     if (planes < 1) return CBCT_ERR_NOMEM;
     *out = (g->d.vol_nz + planes - 1) / planes;
+    return CBCT_OK;
+}
+
+void cbct_prof_begin(cbct_geom *g, int kernel, cudaStream_t st)
+{
+    if (!g->profiling) return;
+    cudaEvent_t a = nullptr, b = nullptr;
+    if (cudaEventCreate(&a) != cudaSuccess || cudaEventCreate(&b) != cudaSuccess) return;
+    cudaEventRecord(a, st);
+    g->prof[kernel].push_back(std::make_pair(a, b));
+}
+
+void cbct_prof_end(cbct_geom *g, int kernel, cudaStream_t st)
+{
+    if (!g->profiling || g->prof[kernel].empty()) return;
+    cudaEventRecord(g->prof[kernel].back().second, st);
+}
+
+static void prof_clear(cbct_geom *g)
+{
+    for (int k = 0; k < 3; ++k) {
+        for (auto &p : g->prof[k]) { cudaEventDestroy(p.first); cudaEventDestroy(p.second); }
+        g->prof[k].clear();
+    }
+}
+
+extern "C" int cbct_geom_profile(cbct_geom *g, int enable)
+{
+    if (!g) return CBCT_ERR_INVALID_ARG;
+    if (enable) prof_clear(g);
+    g->profiling = enable != 0;
+    return CBCT_OK;
+}
+
+extern "C" int cbct_geom_profile_read(cbct_geom *g, int kernel, double *ms_total, uint64_t *launches)
+{
+    if (!g || kernel < 0 || kernel > 2 || !ms_total || !launches) return CBCT_ERR_INVALID_ARG;
+    double total = 0.0;
+    for (auto &p : g->prof[kernel]) {
+        CBCT_CUDA_TRY(cudaEventSynchronize(p.second));
+        float ms = 0.f;
+        CBCT_CUDA_TRY(cudaEventElapsedTime(&ms, p.first, p.second));
+        total += ms;
+    }
+    *ms_total = total;
+    *launches = g->prof[kernel].size();
     return CBCT_OK;
 }
 

@@ -10,6 +10,7 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <utility>
 #include <vector>
 
 #include "../../include/cbct.h"
@@ -64,6 +65,9 @@ struct cbct_geom {
     cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
     uint64_t launches = 0;
     int64_t sample_count = -1;
+    // optional per-launch event pairs of the three main kernels (cbct_geom_profile)
+    bool profiling = false;
+    std::vector<std::pair<cudaEvent_t, cudaEvent_t>> prof[3];
     // symmetries of the geometry the gather adjoint may exploit (cbct_geom.cu):
     int sym_rot = 1;        // 4 / 2 / 1: views i and i + n/sym_rot see the grid rotated by 360/sym_rot deg
     bool sym_mirror_z = false;  // volume and detector symmetric under z -> -z
@@ -89,6 +93,9 @@ int cbct_plan_slab_planes(const cbct_geom *g, int channels);  // planes per z-sl
 
 // --- kernel launchers; all enqueue on `st` ----------------------------------
 int cbct_check_launch(cbct_geom *g, const char *what);
+// bracket a main-kernel launch with an event pair when profiling is on (cbct_geom.cu)
+void cbct_prof_begin(cbct_geom *g, int kernel, cudaStream_t st);
+void cbct_prof_end(cbct_geom *g, int kernel, cudaStream_t st);
 // quad-pack: src[C][nz_src][ny][nx] planes [r.z0, r.z1) -> dst[C][pz][py][px] float4 cells (cbct_fp.cu)
 int cbct_launch_pack_volume(cbct_geom *g, const RayGeom &r, const float *src, float4 *dst, int channels,
                             size_t src_channel_stride, int src_z_origin, cudaStream_t st);
