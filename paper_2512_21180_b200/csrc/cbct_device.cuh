@@ -19,6 +19,7 @@
 // and no error accumulates along the ray (DESIGN.md s.6, precision plan).
 struct Ray {
     float ax, ay, az;  // anchor sample position minus 1/2, padded index coordinates
+    float bx, by, bz;  // anchor sample position itself (rounded separately from fp64)
     float dx, dy, dz;  // position increment per sample
     float kf0;         // first sample index relative to the anchor
     int n;             // number of samples to visit (0 = ray misses the slab)
@@ -59,6 +60,7 @@ __device__ __forceinline__ Ray cbct_ray_setup(const RayGeom &G, double c, double
     cbct_clip_axis(oz, dz, CBCT_PAD - 1.0, CBCT_PAD + (double)(G.z1 - G.z0), tmin, tmax, hit);
     r.n = 0;
     r.ax = r.ay = r.az = 1.f;
+    r.bx = r.by = r.bz = 1.5f;
     r.dx = r.dy = r.dz = 0.f;
     r.kf0 = 0.f;
     if (!hit || !(tmin < tmax)) return r;
@@ -72,6 +74,9 @@ __device__ __forceinline__ Ray cbct_ray_setup(const RayGeom &G, double c, double
     r.ax = (float)(ox + tm * dx - 0.5);
     r.ay = (float)(oy + tm * dy - 0.5);
     r.az = (float)(oz + tm * dz - 0.5);
+    r.bx = (float)(ox + tm * dx);
+    r.by = (float)(oy + tm * dy);
+    r.bz = (float)(oz + tm * dz);
     r.dx = (float)(G.step * dx);
     r.dy = (float)(G.step * dy);
     r.dz = (float)(G.step * dz);

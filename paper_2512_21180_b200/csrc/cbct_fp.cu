@@ -12,17 +12,15 @@
 // LDG.32.  The packed buffer carries a zero border of CBCT_PAD cells, which
 // implements the zero-extension boundary rule R4 with no bounds test in the
 // loop.  CB channels share the position / weight arithmetic of a sample.
-#include <stdlib.h>
-
 #include "cbct_device.cuh"
 
 // Position of cell jx inside its row: the cell keeps its 128-byte line (8 cells) but
-// rotates inside it by a (jy, jz)-dependent amount, so that neighbouring rows and
-// planes put the same jx on different L1 data banks (a quarter-warp's LDG.128 reads
+// rotates inside it by a jy-dependent amount, so that neighbouring rows put the
+// same jx on different L1 data banks (a quarter-warp's LDG.128 reads
 // ~5 distinct cells of a 2-D patch; un-swizzled, equal jx in different rows collide).
-__device__ __forceinline__ int cbct_swizzle(int jx, int jy, int jz, int swy, int swz)
+__device__ __forceinline__ int cbct_swizzle(int jx, int jy, int swy)
 {
-    return (jx & ~7) | ((jx + swy * jy + swz * jz) & 7);
+    return (jx & ~7) | ((jx + swy * jy) & 7);
 }
 
 // ---------------------------------------------------------------------------
@@ -55,7 +53,7 @@ pack_volume_kernel(const float *__restrict__ src, float4 *__restrict__ dst, cons
                 if (okx1) q.w = __ldg(r + x1);
             }
         }
-        d[(size_t)row * G.px + cbct_swizzle(jx, jy, jz, G.swy, G.swz)] = q;
+        d[(size_t)row * G.px + cbct_swizzle(jx, jy, G.swy)] = q;
     }
 }
 
@@ -67,23 +65,41 @@ pack_volume_kernel(const float *__restrict__ src, float4 *__restrict__ dst, cons
 
 __device__ __forceinline__ float lerpf(float a, float b, float t) { return fmaf(t, b - a, a); }
 
-__device__ __forceinline__ float quad_sample(const float4 *__restrict__ p0, const float4 *__restrict__ p1, float fx,
-                                             float fy, float fz)
+// One sample position: the two cell addresses (planes jz and jz + 1) and the three
+// interpolation fractions.  Per axis: pm = fma(kf, d, a) is p - 1/2; y = pm + MAGIC
+// rounds it to the cell index j (held in the low mantissa bits of y); the fraction
+// p - j = fma(kf, d, b - j) is evaluated from the anchor b itself (b - j is exact),
+// so no separate + 1/2.  The cell address uses the raw bits of y: the magic offset
+// contributes the constant `kfold` (mod 2^32), subtracted once.
+struct Sample {
+    const float4 *p0, *p1;
+    float fx, fy, fz;
+};
+
+__device__ __forceinline__ Sample locate(const float4 *__restrict__ packed, const Ray &r, float kf, unsigned py,
+                                         unsigned px, unsigned swy, unsigned kfold, unsigned plane)
 {
-    float4 q0 = __ldg(p0), q1 = __ldg(p1);
-    float b0 = lerpf(lerpf(q0.x, q0.y, fx), lerpf(q0.z, q0.w, fx), fy);
-    float b1 = lerpf(lerpf(q1.x, q1.y, fx), lerpf(q1.z, q1.w, fx), fy);
-    return lerpf(b0, b1, fz);
+    Sample s;
+    const float yx = fmaf(kf, r.dx, r.ax) + CBCT_MAGIC;
+    const float yy = fmaf(kf, r.dy, r.ay) + CBCT_MAGIC;
+    const float yz = fmaf(kf, r.dz, r.az) + CBCT_MAGIC;
+    s.fx = fmaf(kf, r.dx, r.bx - (yx - CBCT_MAGIC));
+    s.fy = fmaf(kf, r.dy, r.by - (yy - CBCT_MAGIC));
+    s.fz = fmaf(kf, r.dz, r.bz - (yz - CBCT_MAGIC));
+    const unsigned ux = __float_as_uint(yx), uy = __float_as_uint(yy), uz = __float_as_uint(yz);
+    const unsigned row = (uz * py + uy) * px + (ux & 0x3FFFF8u);
+    const unsigned idx = row + ((uy * swy + ux) & 7u) - kfold;
+    s.p0 = packed + idx;
+    s.p1 = s.p0 + plane;
+    return s;
 }
 
-// Addresses of the cells (jx, jy, jz) and (jx, jy, jz + 1) of the packed slab.
-__device__ __forceinline__ void cell_pointers(const float4 *__restrict__ packed, const RayGeom &G, int jx, int jy, int jz,
-                                              const float4 *&p0, const float4 *&p1)
+__device__ __forceinline__ float quad_sample(const Sample &s, size_t off)
 {
-    const int row = (jz * G.py + jy) * G.px + (jx & ~7);
-    const int t = jx + G.swy * jy + G.swz * jz;
-    p0 = packed + (row + (t & 7));
-    p1 = packed + (row + G.px * G.py + ((t + G.swz) & 7));
+    const float4 q0 = __ldg(s.p0 + off), q1 = __ldg(s.p1 + off);
+    const float b0 = lerpf(lerpf(q0.x, q0.y, s.fx), lerpf(q0.z, q0.w, s.fx), s.fy);
+    const float b1 = lerpf(lerpf(q1.x, q1.y, s.fx), lerpf(q1.z, q1.w, s.fx), s.fy);
+    return lerpf(b0, b1, s.fz);
 }
 
 // CB channels per thread; a warp covers TU x (32 / TU) pixels; CTA = 16 x 16 pixels.
@@ -102,41 +118,26 @@ fp_kernel(const float4 *__restrict__ packed, float *__restrict__ sino, const __g
     if (iu >= G.nu || iv >= G.nv) return;
     const int view = blockIdx.y;
     const Ray r = cbct_ray_setup(G, V.cs[view].x, V.cs[view].y, iu, iv);
+    const unsigned py = G.py, px = G.px, swy = G.swy, plane = G.px * G.py;
+    const unsigned kfold = (CBCT_MAGIC_BITS * (py + 1u)) * px;  // magic bits of jz, jy folded through the row formula
     float acc[CB], acc2[CB];
 #pragma unroll
     for (int c = 0; c < CB; ++c) acc[c] = acc2[c] = 0.f;
     float kf = r.kf0;
     int it = 0;
     for (; it + 1 < r.n; it += 2, kf += 2.0f) {
-        int jx, jy, jz, kx, ky, kz;
-        float fx, fy, fz, gx, gy, gz;
-        cbct_cell_frac(fmaf(kf, r.dx, r.ax), jx, fx);
-        cbct_cell_frac(fmaf(kf, r.dy, r.ay), jy, fy);
-        cbct_cell_frac(fmaf(kf, r.dz, r.az), jz, fz);
-        const float kg = kf + 1.0f;
-        cbct_cell_frac(fmaf(kg, r.dx, r.ax), kx, gx);
-        cbct_cell_frac(fmaf(kg, r.dy, r.ay), ky, gy);
-        cbct_cell_frac(fmaf(kg, r.dz, r.az), kz, gz);
-        const float4 *p0, *p1, *q0, *q1;
-        cell_pointers(packed, G, jx, jy, jz, p0, p1);
-        cell_pointers(packed, G, kx, ky, kz, q0, q1);
+        const Sample s0 = locate(packed, r, kf, py, px, swy, kfold, plane);
+        const Sample s1 = locate(packed, r, kf + 1.0f, py, px, swy, kfold, plane);
 #pragma unroll
         for (int c = 0; c < CB; ++c) {
-            acc[c] += quad_sample(p0 + c * packed_cstride, p1 + c * packed_cstride, fx, fy, fz);
-            acc2[c] += quad_sample(q0 + c * packed_cstride, q1 + c * packed_cstride, gx, gy, gz);
+            acc[c] += quad_sample(s0, c * packed_cstride);
+            acc2[c] += quad_sample(s1, c * packed_cstride);
         }
     }
     if (it < r.n) {
-        int jx, jy, jz;
-        float fx, fy, fz;
-        cbct_cell_frac(fmaf(kf, r.dx, r.ax), jx, fx);
-        cbct_cell_frac(fmaf(kf, r.dy, r.ay), jy, fy);
-        cbct_cell_frac(fmaf(kf, r.dz, r.az), jz, fz);
-        const float4 *p0, *p1;
-        cell_pointers(packed, G, jx, jy, jz, p0, p1);
+        const Sample s0 = locate(packed, r, kf, py, px, swy, kfold, plane);
 #pragma unroll
-        for (int c = 0; c < CB; ++c)
-            acc[c] += quad_sample(p0 + c * packed_cstride, p1 + c * packed_cstride, fx, fy, fz);
+        for (int c = 0; c < CB; ++c) acc[c] += quad_sample(s0, c * packed_cstride);
     }
     const float delta = (float)G.delta;
     const size_t o = ((size_t)(view0 + view) * G.nv + iv) * G.nu + iu;
@@ -171,10 +172,7 @@ static int launch_fp_cb(cbct_geom *g, const RayGeom &r, const ViewChunk &vc, int
 {
     dim3 grid((r.nu + FP_CTA_U - 1) / FP_CTA_U, nviews, (r.nv + FP_CTA_V - 1) / FP_CTA_V);
     cbct_prof_begin(g, CBCT_KERNEL_FP, st);
-    static const int tu = getenv("CBCT_FP_TU") ? atoi(getenv("CBCT_FP_TU")) : 8;  // TODO(tuning): remove
-    if (tu == 4) fp_kernel<CB, 4><<<grid, FP_CTA_U * FP_CTA_V, 0, st>>>(packed, sino, r, vc, view0, accumulate, pstride, sstride);
-    else if (tu == 16) fp_kernel<CB, 16><<<grid, FP_CTA_U * FP_CTA_V, 0, st>>>(packed, sino, r, vc, view0, accumulate, pstride, sstride);
-    else fp_kernel<CB, 8><<<grid, FP_CTA_U * FP_CTA_V, 0, st>>>(packed, sino, r, vc, view0, accumulate, pstride, sstride);
+    fp_kernel<CB, 8><<<grid, FP_CTA_U * FP_CTA_V, 0, st>>>(packed, sino, r, vc, view0, accumulate, pstride, sstride);
     cbct_prof_end(g, CBCT_KERNEL_FP, st);
     return cbct_check_launch(g, "fp_kernel");
 }
@@ -184,7 +182,6 @@ int cbct_launch_fp(cbct_geom *g, const RayGeom &r, const float4 *packed, float *
 {
     const size_t pstride = cbct_packed_volume_cells(r);
     const size_t sstride = (size_t)g->d.n_views * r.nv * r.nu;
-    static const int cbmax = getenv("CBCT_FP_CB") ? atoi(getenv("CBCT_FP_CB")) : 4;  // TODO(tuning): remove
     ViewChunk vc;  // 8 KB; copied into the launch's parameter buffer at launch time
     for (int view0 = 0; view0 < g->d.n_views; view0 += CBCT_VIEWS_PER_LAUNCH) {
         int n = g->d.n_views - view0;
@@ -195,8 +192,8 @@ int cbct_launch_fp(cbct_geom *g, const RayGeom &r, const float4 *packed, float *
             int left = channels - c, rc;
             const float4 *p = packed + c * pstride;
             float *s = sino + c * sstride;
-            if (left >= 4 && cbmax >= 4) { rc = launch_fp_cb<4>(g, r, vc, n, view0, p, s, accumulate, pstride, sstride, st); c += 4; }
-            else if (left >= 2 && cbmax >= 2) { rc = launch_fp_cb<2>(g, r, vc, n, view0, p, s, accumulate, pstride, sstride, st); c += 2; }
+            // 2 channels per thread measured best at 256^3 (4 lowers occupancy and L1 hit rate)
+            if (left >= 2) { rc = launch_fp_cb<2>(g, r, vc, n, view0, p, s, accumulate, pstride, sstride, st); c += 2; }
             else { rc = launch_fp_cb<1>(g, r, vc, n, view0, p, s, accumulate, pstride, sstride, st); c += 1; }
             if (rc) return rc;
         }

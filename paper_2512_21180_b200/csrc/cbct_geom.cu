@@ -3,7 +3,6 @@
 // converts every length to voxel units, plans z-slabs, and counts in-support
 // samples analytically.  Geometry: PAPER.md:61; readings R2-R7 (DESIGN.md s.3).
 #include <math.h>
-#include <stdlib.h>
 #include <string.h>
 
 #include <new>
@@ -142,8 +141,7 @@ RayGeom cbct_make_raygeom(const cbct_geom *g, int z0, int z1)
     r.px = (d.vol_nx + 2 * CBCT_PAD + 7) & ~7;  // row pitch: whole 128-byte lines of 8 float4 cells
     r.py = d.vol_ny + 2 * CBCT_PAD;
     r.pz = (z1 - z0) + 2 * CBCT_PAD;
-    r.swy = getenv("CBCT_SWY") ? atoi(getenv("CBCT_SWY")) : CBCT_SWIZZLE_Y;  // TODO(tuning): remove
-    r.swz = getenv("CBCT_SWZ") ? atoi(getenv("CBCT_SWZ")) : CBCT_SWIZZLE_Z;
+    r.swy = CBCT_SWIZZLE_Y;
     return r;
 }
 
