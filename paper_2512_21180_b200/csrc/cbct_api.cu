@@ -117,7 +117,10 @@ extern "C" int cbct_fp(const cbct_geom *gc, const float *vol, float *sino, int32
         rc = ensure(&g->ws_stage, &g->ws_stage_bytes, stage_elems * nbuf * sizeof(float));
         if (rc) return rc;
     }
-    if (n_slabs > 1) {  // the copy stream starts after everything already queued on `st`
+    if (n_slabs > 1) {
+        // every slab adds its part (only into the detector rows its shadow covers) to a zeroed sinogram
+        CBCT_CUDA_TRY(cudaMemsetAsync(d_sino, 0, cx.nsino * channels * sizeof(float), st));
+        // the copy stream starts after everything already queued on `st`
         CBCT_CUDA_TRY(cudaEventRecord(g->ev[0], st));
         CBCT_CUDA_TRY(cudaStreamWaitEvent(g->copy_stream, g->ev[0], 0));
     }
@@ -144,7 +147,7 @@ extern "C" int cbct_fp(const cbct_geom *gc, const float *vol, float *sino, int32
             CBCT_CUDA_TRY(cudaEventRecord(g->ev[b], cs));
             CBCT_CUDA_TRY(cudaStreamWaitEvent(st, g->ev[b], 0));
         }
-        rc = cbct_launch_fp(g, r, buf, d_sino, channels, s > 0, st);
+        rc = cbct_launch_fp(g, r, buf, d_sino, channels, n_slabs > 1, st);
         if (rc) return rc;
         if (n_slabs > 1) CBCT_CUDA_TRY(cudaEventRecord(g->ev[2 + b], st));
     }

@@ -107,14 +107,14 @@ template <int CB, int TU>
 __global__ void __launch_bounds__(FP_CTA_U *FP_CTA_V)
 fp_kernel(const float4 *__restrict__ packed, float *__restrict__ sino, const __grid_constant__ RayGeom G,
           const __grid_constant__ ViewChunk V, int view0, int accumulate, size_t packed_cstride,
-          size_t sino_cstride)
+          size_t sino_cstride, int band0)
 {
     constexpr int TV = 32 / TU, WU = FP_CTA_U / TU;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int iu = blockIdx.x * FP_CTA_U + (warp % WU) * TU + (lane % TU);
     // grid = (u tiles, views, v bands): CTAs in flight share a band of detector rows, i.e. a thin
     // z-slab of the volume, which then stays L2-resident across all views
-    const int iv = blockIdx.z * FP_CTA_V + (warp / WU) * TV + (lane / TU);
+    const int iv = (band0 + blockIdx.z) * FP_CTA_V + (warp / WU) * TV + (lane / TU);
     if (iu >= G.nu || iv >= G.nv) return;
     const int view = blockIdx.y;
     const Ray r = cbct_ray_setup(G, V.cs[view].x, V.cs[view].y, iu, iv);
@@ -168,11 +168,12 @@ int cbct_launch_pack_volume(cbct_geom *g, const RayGeom &r, const float *src, fl
 template <int CB>
 static int launch_fp_cb(cbct_geom *g, const RayGeom &r, const ViewChunk &vc, int nviews, int view0,
                         const float4 *packed, float *sino, int accumulate, size_t pstride, size_t sstride,
-                        cudaStream_t st)
+                        int band0, int nbands, cudaStream_t st)
 {
-    dim3 grid((r.nu + FP_CTA_U - 1) / FP_CTA_U, nviews, (r.nv + FP_CTA_V - 1) / FP_CTA_V);
+    dim3 grid((r.nu + FP_CTA_U - 1) / FP_CTA_U, nviews, nbands);
     cbct_prof_begin(g, CBCT_KERNEL_FP, st);
-    fp_kernel<CB, 8><<<grid, FP_CTA_U * FP_CTA_V, 0, st>>>(packed, sino, r, vc, view0, accumulate, pstride, sstride);
+    fp_kernel<CB, 8><<<grid, FP_CTA_U * FP_CTA_V, 0, st>>>(packed, sino, r, vc, view0, accumulate, pstride, sstride,
+                                                           band0);
     cbct_prof_end(g, CBCT_KERNEL_FP, st);
     return cbct_check_launch(g, "fp_kernel");
 }
@@ -182,6 +183,23 @@ int cbct_launch_fp(cbct_geom *g, const RayGeom &r, const float4 *packed, float *
 {
     const size_t pstride = cbct_packed_volume_cells(r);
     const size_t sstride = (size_t)g->d.n_views * r.nv * r.nu;
+    // Detector rows a partial slab can reach (its shadow): a ray of height coordinate v is at
+    // z = lambda v with lambda = U / sdd, U within [sid - R, sid + R] over the grid's xy extent;
+    // only the bands of 16 rows meeting that range are launched.  A caller that launches partial
+    // slabs must have zeroed the sinogram and pass accumulate != 0.
+    int band0 = 0, nbands = (r.nv + FP_CTA_V - 1) / FP_CTA_V;
+    if (r.z0 > 0 || r.z1 < r.nz) {
+        const double R = sqrt(r.cx * r.cx + r.cy * r.cy) + 0.5 * sqrt((double)(r.nx + 1) * (r.nx + 1) + (double)(r.ny + 1) * (r.ny + 1));
+        const double lmin = (r.sid - R) / (r.sid + r.idd), lmax = (r.sid + R) / (r.sid + r.idd);
+        const double za = r.cz + (r.z0 - 1.0 - 0.5 * (r.nz - 1)), zb = r.cz + (r.z1 - 0.5 * (r.nz - 1));
+        const double vlo = za <= 0.0 ? za / lmin : za / lmax, vhi = zb >= 0.0 ? zb / lmin : zb / lmax;
+        int iv_lo = (int)floor((vlo - r.v0) / r.dv) - 1, iv_hi = (int)ceil((vhi - r.v0) / r.dv) + 1;
+        if (iv_lo < 0) iv_lo = 0;
+        if (iv_hi > r.nv - 1) iv_hi = r.nv - 1;
+        if (iv_lo > iv_hi) return CBCT_OK;  // the slab's shadow misses the detector
+        band0 = iv_lo / FP_CTA_V;
+        nbands = iv_hi / FP_CTA_V - band0 + 1;
+    }
     ViewChunk vc;  // 8 KB; copied into the launch's parameter buffer at launch time
     for (int view0 = 0; view0 < g->d.n_views; view0 += CBCT_VIEWS_PER_LAUNCH) {
         int n = g->d.n_views - view0;
@@ -193,8 +211,8 @@ int cbct_launch_fp(cbct_geom *g, const RayGeom &r, const float4 *packed, float *
             const float4 *p = packed + c * pstride;
             float *s = sino + c * sstride;
             // 2 channels per thread measured best at 256^3 (4 lowers occupancy and L1 hit rate)
-            if (left >= 2) { rc = launch_fp_cb<2>(g, r, vc, n, view0, p, s, accumulate, pstride, sstride, st); c += 2; }
-            else { rc = launch_fp_cb<1>(g, r, vc, n, view0, p, s, accumulate, pstride, sstride, st); c += 1; }
+            if (left >= 2) { rc = launch_fp_cb<2>(g, r, vc, n, view0, p, s, accumulate, pstride, sstride, band0, nbands, st); c += 2; }
+            else { rc = launch_fp_cb<1>(g, r, vc, n, view0, p, s, accumulate, pstride, sstride, band0, nbands, st); c += 1; }
             if (rc) return rc;
         }
     }

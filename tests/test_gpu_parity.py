@@ -283,3 +283,70 @@ def test_config3_pyramid_sampled(cbct, oracle_mod, name):
     assert rel_l2(gsel, r) <= 1e-5, rel_l2(gsel, r)
     floor = 1e-3 * float(np.max(np.abs(r)))
     assert np.max(np.abs(gsel - r) / np.maximum(np.abs(r), floor)) <= 1e-4
+
+
+def _sampled_checks(oracle_mod, og, vol_c, sino_c, Ax_c, Aty_c, F_c, seeds, n_rays=2000, n_adj=48, n_fdk=2000):
+    """One channel: sampled forward rays, adjoint voxels and FDK voxels against the oracle."""
+    v64, s64 = vol_c[None].astype(np.float64), sino_c[None].astype(np.float64)
+    ridx = synth.sample_indices(seeds[0], Ax_c.size, n_rays)
+    r = oracle_mod.fp_rays(og, v64, ridx)[0]
+    gsel = Ax_c.reshape(-1)[ridx]
+    ra = oracle_mod.fp_rays(og, np.abs(v64), ridx)[0]
+    den = np.maximum(np.maximum(np.abs(r), 0.1 * ra), 1e-3 * float(np.max(np.abs(r))))   # R16 / R16b
+    assert rel_l2(gsel, r) <= 1e-5, rel_l2(gsel, r)
+    assert float(np.max(np.abs(gsel - r) / den)) <= 1e-4
+    vidx = synth.sample_indices(seeds[1], vol_c.size, n_adj)
+    r = oracle_mod.bp_adjoint_voxels(og, s64, vidx)[0]
+    assert rel_l2(Aty_c.reshape(-1)[vidx], r) <= 1e-4
+    vidx = synth.sample_indices(seeds[2], vol_c.size, n_fdk)
+    r = oracle_mod.bp_fdk_voxels(og, s64, vidx)[0]
+    gsel = F_c.reshape(-1)[vidx]
+    assert rel_l2(gsel, r) <= 1e-5, rel_l2(gsel, r)
+    floor = 1e-3 * float(np.max(np.abs(r)))
+    assert np.max(np.abs(gsel - r) / np.maximum(np.abs(r), floor)) <= 1e-4
+
+
+def test_config4_multichannel_sampled(cbct, oracle_mod):
+    """Config 4 as bench.py launches it: 256^3, 8 channels (phantom + 7 signed noise fields), 400 views,
+    one call per operator over all channels.  Channels 0, 1 and 7 are checked on sampled outputs."""
+    cfg = synth.CONFIGS["multichannel_256"]
+    kw = synth.geom_kwargs(cfg)
+    og = oracle_mod.Geom(**kw)
+    vol, sino = synth.make_volume(cfg), synth.make_sinogram(cfg)
+    Ax, Aty, F = run_fp(cbct, kw, vol), run_adj(cbct, kw, sino), run_fdk(cbct, kw, sino)
+    for c in (0, 1, 7):
+        _sampled_checks(oracle_mod, og, vol[c], sino[c], Ax[c], Aty[c], F[c], (41 + c, 51 + c, 61 + c),
+                        n_rays=800, n_adj=16, n_fdk=800)
+    # channel independence at full size: channel 3 alone gives the same bits as channel 3 of the batch
+    one = run_fp(cbct, kw, vol[3:4])
+    assert np.array_equal(one[0], Ax[3])
+
+
+def test_config5_large_streamed_sampled(cbct, oracle_mod):
+    """Config 5: 512^3 at 1 mm, 4 channels, 720 views, 512^2 offset detector, volume in pinned HOST memory
+    under a 1 GiB work-set cap (forces the z-slab streaming path, A5).  Channel 0 (phantom) and channel 1
+    (noise) are checked on sampled outputs; the fp32 adjoint identity is checked on channel 0."""
+    cfg = synth.CONFIGS["large_512"]
+    kw = synth.geom_kwargs(cfg)
+    C = cfg["channels"]
+    g = cbct.Geometry(**kw, max_workset_bytes=1 << 30)
+    assert g.num_slabs(C) > 8
+    og = oracle_mod.Geom(**kw)
+    vol = torch.from_numpy(synth.make_volume(cfg)).pin_memory()
+    sino = torch.from_numpy(synth.make_sinogram(cfg)).cuda()
+    Ax = torch.empty((C,) + g.sino_shape, device="cuda")
+    g.fp(vol, Ax, C)
+    out = torch.empty((C,) + g.vol_shape).pin_memory()
+    g.bp_adjoint(sino, out, C)
+    torch.cuda.synchronize()
+    Aty = out.numpy().copy()
+    g.bp_fdk(sino, out, C)
+    torch.cuda.synchronize()
+    F = out.numpy()
+    Ax_h, sino_h, vol_h = Ax.cpu().numpy(), sino.cpu().numpy(), vol.numpy()
+    for c in (0, 1):
+        _sampled_checks(oracle_mod, og, vol_h[c], sino_h[c], Ax_h[c], Aty[c], F[c], (71 + c, 81 + c, 91 + c),
+                        n_rays=1000, n_adj=12, n_fdk=1000)
+    lhs = float(np.sum(Ax_h[0].astype(np.float64) * sino_h[0]))
+    rhs = float(np.sum(vol_h[0].astype(np.float64) * Aty[0]))
+    assert abs(lhs - rhs) / abs(lhs) <= 1e-5, (lhs, rhs)
