@@ -28,8 +28,9 @@ UNIT = "Gsamples/s"
 
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of each kernel at the default workload,
-# from the ncu --set full capture summarised in profiles/ (None = not captured for this build).
-NCU_DRAM_BYTES_PER_LAUNCH = {"fp_kernel": None, "adjoint_gather_kernel": None, "fdk_kernel": None}
+# from the ncu --set full capture summarised in profiles/r1_final.md (multichannel_256; fp and adjoint launches
+# carry 2 channels, fdk launches 1).  Reported only for that workload.
+NCU_DRAM_BYTES_PER_LAUNCH = {"fp_kernel": 0.748e9, "adjoint_gather_kernel": 2.230e9, "fdk_kernel": 0.213e9}
 
 
 def peaks():
@@ -128,6 +129,9 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="multichannel_256")
     ap.add_argument("--channels", type=int, default=0, help="override the workload's channel count")
+    ap.add_argument("--cap-gib", type=float, default=-1.0,
+                    help="max_workset_bytes in GiB (0 = none); default: 1 for large_512 (BASELINE.json config 5), else 0. "
+                         "With a cap the volumes live in pinned HOST memory and stream through z-slabs")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
@@ -155,16 +159,19 @@ def main():
 
     C = cfg["channels"]
     kw = synth.geom_kwargs(cfg)
-    g = cbct.Geometry(**kw)
+    cap_gib = args.cap_gib if args.cap_gib >= 0 else (1.0 if cfg["name"] == "large_512" else 0.0)
+    streamed = cap_gib > 0
+    g = cbct.Geometry(**kw, max_workset_bytes=int(cap_gib * (1 << 30)))
     n_samples = g.count_samples()                    # per channel, analytic fp64 (host)
     n_vv = g.n_vol * cfg["n_views"]                  # voxel-views per channel
     # every rank works on its own batch of C channels (weak scaling, no data-path collective)
     vol_h = synth.make_volume(cfg)
     sino_h = synth.make_sinogram(cfg)
-    vol = torch.from_numpy(vol_h).cuda()
+    # resident case: everything in HBM; streamed case: volumes in pinned host memory (A5)
+    vol = torch.from_numpy(vol_h).pin_memory() if streamed else torch.from_numpy(vol_h).cuda()
     sino_in = torch.from_numpy(sino_h).cuda()
     sino_out = torch.empty_like(sino_in)
-    vol_out = torch.empty_like(vol)
+    vol_out = torch.empty_like(vol).pin_memory() if streamed else torch.empty_like(vol)
 
     def step(ev=None):
         if ev:
@@ -200,7 +207,7 @@ def main():
 
     # end to end through the C ABI with HOST (pinned) buffers: copies inside the timed region
     e2e = None
-    if not args.no_e2e:
+    if not args.no_e2e and not streamed:
         hv, hs = torch.from_numpy(vol_h).pin_memory(), torch.from_numpy(sino_h).pin_memory()
         hso, hvo = torch.empty_like(hs).pin_memory(), torch.empty_like(hv).pin_memory()
 
@@ -239,6 +246,12 @@ def main():
     fwd = world * C * n_samples / (t_fp * 1e-3) / 1e9
     adj_vv = world * C * n_vv / (t_adj * 1e-3) / 1e9
     fdk_vv = world * C * n_vv / (t_fdk * 1e-3) / 1e9
+    if streamed and not args.no_e2e:
+        # the timed region already copies the volumes host <-> device inside every call
+        e2e = {"value": fwd, "unit": UNIT, "h2d_bytes_per_step": int(vol_h.nbytes),
+               "d2h_bytes_per_step": int(2 * vol_h.nbytes), "ms_per_step": t_total, "fp_ms": t_fp,
+               "note": "streamed workload: volumes are pinned HOST buffers in the main timed region; "
+                       "sinograms stay in HBM"}
     # Roofline of the dominant kernel (DESIGN.md s.7).  Algorithmic on-SM bytes per unit:
     # forward 32 B per sample (8 taps x 4 B through L1), adjoint 64 B per sample (the scatter form's
     # 8 tap read-modify-writes; the gather does less), FDK 16 B per voxel-view; peak =
@@ -259,7 +272,7 @@ def main():
     dom = max(per_kernel, key=lambda k: kern[k][0])
     hbm_alg = C * 4.0 * (g.n_vol + g.n_sino) * args.steps / kern[dom][1]
     roofline = {"kernel": dom, "bound": "l1", "achieved": per_kernel[dom]["achieved_gbs"], "peak": l1_peak,
-                "unit": "GB/s", "frac": per_kernel[dom]["frac"], "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get(dom),
+                "unit": "GB/s", "frac": per_kernel[dom]["frac"], "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get(dom) if (cfg["name"] == "multichannel_256" and C == 8) else None,
                 "peak_source": f"derived: 148 SM x 128 B/clk x {sm_hz / 1e6:.0f} MHz (L1 data path; MEASURED_PEAKS.json "
                                "has no L1 figure; HBM is not the bound, see hbm_frac)",
                 "traffic_source": "profiles/r1_final.md (ncu --set full, dram__bytes_read.sum + dram__bytes_write.sum)",
@@ -274,6 +287,8 @@ def main():
             "config": {"workload": cfg["name"], "volume": [cfg["vol_nz"], cfg["vol_ny"], cfg["vol_nx"]],
                        "vox_mm": cfg["vox_mm"], "views": cfg["n_views"], "detector": [cfg["det_nv"], cfg["det_nu"]],
                        "channels": C, "step_vox": cfg["step_vox"], "l2": "inputs larger than L2 (no flush)",
+                       "max_workset_gib": cap_gib, "slabs": g.num_slabs(C),
+                       "volumes": "pinned host memory, streamed by z-slabs" if streamed else "HBM-resident",
                        "step": "cbct_fp + cbct_bp_adjoint + cbct_bp_fdk over all channels",
                        "sharding": "each rank runs its own C-channel batch; no data-path collective"},
             "backprojection": {"adjoint_gvoxel_views_per_s": adj_vv, "adjoint_gsamples_per_s":
