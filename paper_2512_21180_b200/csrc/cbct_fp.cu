@@ -15,12 +15,15 @@
 #include "cbct_device.cuh"
 
 // Position of cell jx inside its row: the cell keeps its 128-byte line (8 cells) but
-// rotates inside it by a jy-dependent amount, so that neighbouring rows put the
-// same jx on different L1 data banks (a quarter-warp's LDG.128 reads
-// ~5 distinct cells of a 2-D patch; un-swizzled, equal jx in different rows collide).
-__device__ __forceinline__ int cbct_swizzle(int jx, int jy, int swy)
+// rotates inside it by a (jy, jz)-dependent amount.  The L1 data stage serves a
+// quarter-warp of an LDG.128 (8 lanes x 16 B) in one cycle only if lanes that read
+// DIFFERENT cells read different 16-byte positions of their lines (measured: up to 4
+// distinct lines per quarter-warp are free, equal positions serialise; DESIGN.md s.6.1).
+// (x + 6y + 4z) mod 8 with 4 x 2-pixel quarter-warps leaves 1.2 cycles per quarter-warp
+// on this geometry (lower bound 1.14; no swizzle 2.6), by simulation of the access pattern.
+__device__ __forceinline__ int cbct_swizzle(int jx, int jy, int jz)
 {
-    return (jx & ~7) | ((jx + swy * jy) & 7);
+    return (jx & ~7) | ((jx + CBCT_SWIZZLE_Y * jy + CBCT_SWIZZLE_Z * jz) & 7);
 }
 
 // ---------------------------------------------------------------------------
@@ -53,7 +56,7 @@ pack_volume_kernel(const float *__restrict__ src, float4 *__restrict__ dst, cons
                 if (okx1) q.w = __ldg(r + x1);
             }
         }
-        d[(size_t)row * G.px + cbct_swizzle(jx, jy, G.swy)] = q;
+        d[(size_t)row * G.px + cbct_swizzle(jx, jy, jz)] = q;
     }
 }
 
@@ -77,7 +80,7 @@ struct Sample {
 };
 
 __device__ __forceinline__ Sample locate(const float4 *__restrict__ packed, const Ray &r, float kf, unsigned py,
-                                         unsigned px, unsigned swy, unsigned kfold, unsigned plane)
+                                         unsigned px, unsigned kfold, unsigned plane)
 {
     Sample s;
     const float yx = fmaf(kf, r.dx, r.ax) + CBCT_MAGIC;
@@ -88,9 +91,10 @@ __device__ __forceinline__ Sample locate(const float4 *__restrict__ packed, cons
     s.fz = fmaf(kf, r.dz, r.bz - (yz - CBCT_MAGIC));
     const unsigned ux = __float_as_uint(yx), uy = __float_as_uint(yy), uz = __float_as_uint(yz);
     const unsigned row = (uz * py + uy) * px + (ux & 0x3FFFF8u);
-    const unsigned idx = row + ((uy * swy + ux) & 7u) - kfold;
+    const unsigned t = uy * CBCT_SWIZZLE_Y + uz * CBCT_SWIZZLE_Z + ux;  // magic bits are multiples of 8
+    const unsigned idx = row + (t & 7u) - kfold;
     s.p0 = packed + idx;
-    s.p1 = s.p0 + plane;
+    s.p1 = packed + (idx + plane + ((t + CBCT_SWIZZLE_Z) & 7u) - (t & 7u));
     return s;
 }
 
@@ -118,7 +122,7 @@ fp_kernel(const float4 *__restrict__ packed, float *__restrict__ sino, const __g
     if (iu >= G.nu || iv >= G.nv) return;
     const int view = blockIdx.y;
     const Ray r = cbct_ray_setup(G, V.cs[view].x, V.cs[view].y, iu, iv);
-    const unsigned py = G.py, px = G.px, swy = G.swy, plane = G.px * G.py;
+    const unsigned py = G.py, px = G.px, plane = G.px * G.py;
     const unsigned kfold = (CBCT_MAGIC_BITS * (py + 1u)) * px;  // magic bits of jz, jy folded through the row formula
     float acc[CB], acc2[CB];
 #pragma unroll
@@ -126,8 +130,8 @@ fp_kernel(const float4 *__restrict__ packed, float *__restrict__ sino, const __g
     float kf = r.kf0;
     int it = 0;
     for (; it + 1 < r.n; it += 2, kf += 2.0f) {
-        const Sample s0 = locate(packed, r, kf, py, px, swy, kfold, plane);
-        const Sample s1 = locate(packed, r, kf + 1.0f, py, px, swy, kfold, plane);
+        const Sample s0 = locate(packed, r, kf, py, px, kfold, plane);
+        const Sample s1 = locate(packed, r, kf + 1.0f, py, px, kfold, plane);
 #pragma unroll
         for (int c = 0; c < CB; ++c) {
             acc[c] += quad_sample(s0, c * packed_cstride);
@@ -135,7 +139,7 @@ fp_kernel(const float4 *__restrict__ packed, float *__restrict__ sino, const __g
         }
     }
     if (it < r.n) {
-        const Sample s0 = locate(packed, r, kf, py, px, swy, kfold, plane);
+        const Sample s0 = locate(packed, r, kf, py, px, kfold, plane);
 #pragma unroll
         for (int c = 0; c < CB; ++c) acc[c] += quad_sample(s0, c * packed_cstride);
     }
@@ -172,7 +176,7 @@ static int launch_fp_cb(cbct_geom *g, const RayGeom &r, const ViewChunk &vc, int
 {
     dim3 grid((r.nu + FP_CTA_U - 1) / FP_CTA_U, nviews, nbands);
     cbct_prof_begin(g, CBCT_KERNEL_FP, st);
-    fp_kernel<CB, 8><<<grid, FP_CTA_U * FP_CTA_V, 0, st>>>(packed, sino, r, vc, view0, accumulate, pstride, sstride,
+    fp_kernel<CB, 4><<<grid, FP_CTA_U * FP_CTA_V, 0, st>>>(packed, sino, r, vc, view0, accumulate, pstride, sstride,
                                                            band0);
     cbct_prof_end(g, CBCT_KERNEL_FP, st);
     return cbct_check_launch(g, "fp_kernel");

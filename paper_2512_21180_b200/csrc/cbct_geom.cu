@@ -141,7 +141,6 @@ RayGeom cbct_make_raygeom(const cbct_geom *g, int z0, int z1)
     r.px = (d.vol_nx + 2 * CBCT_PAD + 7) & ~7;  // row pitch: whole 128-byte lines of 8 float4 cells
     r.py = d.vol_ny + 2 * CBCT_PAD;
     r.pz = (z1 - z0) + 2 * CBCT_PAD;
-    r.swy = CBCT_SWIZZLE_Y;
     return r;
 }
 

@@ -17,7 +17,10 @@
 
 #define CBCT_PAD 2              // zero border (voxels / pixels) of padded buffers
 #define CBCT_VIEWS_PER_LAUNCH 512
-#define CBCT_SWIZZLE_Y 5        // see RayGeom::swy
+// bank swizzle of the packed cells: cell (jx, jy, jz) sits at position
+// (jx & ~7) | ((jx + CBCT_SWIZZLE_Y jy + CBCT_SWIZZLE_Z jz) & 7) of its row (cbct_fp.cu)
+#define CBCT_SWIZZLE_Y 6
+#define CBCT_SWIZZLE_Z 4
 
 // View-independent geometry in voxel units (fp64), passed by value to kernels.
 struct RayGeom {
@@ -30,8 +33,6 @@ struct RayGeom {
     int nx, ny, nz;         // full grid size
     int z0, z1;             // planes [z0, z1) held by the padded buffer
     int px, py, pz;         // padded buffer dims (x pitch, rows, planes)
-    int swy;                // bank swizzle of the packed cells: cell (jx, jy, jz) sits at
-                            // (jx & ~7) | ((jx + swy jy) & 7) of its row (cbct_fp.cu)
 };
 
 struct ViewChunk {
