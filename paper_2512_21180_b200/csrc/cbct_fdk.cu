@@ -54,8 +54,14 @@ pad_sino_kernel(const float *__restrict__ in, float *__restrict__ out, int nu, i
 // ---------------------------------------------------------------------------
 // backprojection kernel
 // ---------------------------------------------------------------------------
-#define FDK_BX 32
-#define FDK_BY 4
+// A warp covers 4 (x) x 8 (y) columns, so a quarter-warp (the unit the L1 data stage serves per
+// cycle for LDG.128) is a compact 4 x 2 patch: its 8 taps fall on ~5.7 distinct pixels within
+// ~8 detector columns instead of ~7.2 pixels over ~11 columns for 8 columns in a row, which
+// halves the 16-byte-position conflicts (profiles/r1_l1_microbench.md; simulated 1.76 -> 1.29
+// cycles per quarter-warp; measured 5.85 -> 5.18 ms).  A row-dependent swizzle of the sinogram
+// (simulated 1.22) cost more address arithmetic than it saved (6.2 ms) and was dropped.
+#define FDK_BX 4
+#define FDK_BY 32
 
 struct FdkViews {
     double2 cs[CBCT_VIEWS_PER_LAUNCH];
