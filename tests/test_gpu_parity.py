@@ -350,3 +350,39 @@ def test_config5_large_streamed_sampled(cbct, oracle_mod):
     lhs = float(np.sum(Ax_h[0].astype(np.float64) * sino_h[0]))
     rhs = float(np.sum(vol_h[0].astype(np.float64) * Aty[0]))
     assert abs(lhs - rhs) / abs(lhs) <= 1e-5, (lhs, rhs)
+
+
+@pytest.mark.parametrize("n_views", [1040, 1037])
+def test_more_views_than_one_launch_chunk(cbct, oracle_mod, n_views):
+    """> 512 views: the kernels take the views in chunks of 512 and accumulate (with 1040 views the
+    rotation-shared backprojectors cross two quarter-turn blocks inside a chunk; 1037 has no rotation)."""
+    kw = dict(synth.geom_kwargs(synth.CONFIGS["tiny"]))
+    kw.update(n_views=n_views, vol_nx=16, vol_ny=16, vol_nz=12, det_nu=20, det_nv=18, det_du_mm=6.0, det_dv_mm=6.0,
+              det_off_u_mm=9.0)
+    rng = np.random.default_rng(5)
+    vol = rng.random((2, 12, 16, 16), dtype=np.float32)
+    sino = rng.random((2, n_views, 18, 20), dtype=np.float32)
+    check_all_three(cbct, oracle_mod, kw, vol, sino, "chunks")
+
+
+def test_outputs_stay_inside_their_buffers(cbct):
+    """compute-sanitizer is closed on this GPU pool, so out-of-bounds writes are looked for directly:
+    every output lives between two guard regions that must come back untouched (ragged sizes, every
+    symmetry class of the backprojectors, resident and z-slab paths)."""
+    G = 4096
+    for over in (dict(), dict(vol_nx=37, vol_ny=29, vol_nz=21, det_nu=50, det_nv=35, n_views=11, vol_cx_mm=5.0),
+                 dict(n_views=10, vol_nx=30, vol_nz=27), dict(n_views=7, det_off_v_mm=3.0)):
+        kw = dict(synth.geom_kwargs(synth.CONFIGS["tiny"]))
+        kw.update(over)
+        for cap in (0, 2500000):
+            g = cbct.Geometry(**kw, max_workset_bytes=cap)
+            C = 3
+            rng = np.random.default_rng(8)
+            vol = dev(rng.random((C,) + g.vol_shape, dtype=np.float32))
+            sino = dev(rng.random((C,) + g.sino_shape, dtype=np.float32))
+            for fn, src, n_out in ((g.fp, vol, C * g.n_sino), (g.bp_adjoint, sino, C * g.n_vol), (g.bp_fdk, sino, C * g.n_vol)):
+                buf = torch.full((n_out + 2 * G,), -7.25, device="cuda", dtype=torch.float32)
+                fn(src, buf[G:G + n_out], C)
+                torch.cuda.synchronize()
+                assert bool((buf[:G] == -7.25).all()) and bool((buf[G + n_out:] == -7.25).all())
+                assert bool(torch.isfinite(buf[G:G + n_out]).all())
