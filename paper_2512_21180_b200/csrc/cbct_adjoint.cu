@@ -66,19 +66,22 @@ interleave_views_kernel(const float *__restrict__ in, float *__restrict__ out, i
     }
 }
 
-#define ADJ_BX 32
-#define ADJ_BY 4
+// A warp covers 8 (x) x 4 (y) voxels of one plane: compact on the detector, so the lanes walk similar
+// (iu, iv) ranges (measured 32.0 -> 29.5 ms per channel against 32 x 1; 4 x 8 and 8 x 2 x 2: 29.8, 29.7).
+#define ADJ_BX 8
+#define ADJ_BY 16
+#define ADJ_BZ 1
 
 template <int NR, int NM, int CB>
-__global__ void __launch_bounds__(ADJ_BX *ADJ_BY)
+__global__ void __launch_bounds__(ADJ_BX *ADJ_BY *ADJ_BZ)
 adjoint_gather_kernel(const float *__restrict__ sinoI, float *__restrict__ vol, const __grid_constant__ AdjGeom G,
                       const __grid_constant__ ViewChunk V, int q0, int accumulate, size_t sino_cstride,
                       size_t vol_cstride, int vol_z_origin)
 {
     const int ix = blockIdx.x * ADJ_BX + threadIdx.x;
     const int iy = blockIdx.y * ADJ_BY + threadIdx.y;
-    const int iz = G.bz0 + blockIdx.z;
-    if (ix >= G.bx || iy >= G.by) return;
+    const int iz = G.bz0 + blockIdx.z * ADJ_BZ + threadIdx.z;
+    if (ix >= G.bx || iy >= G.by || iz >= G.bz1) return;
     const double X = G.x0 + ix, Y = G.y0 + iy, Z = G.z0 + iz;
     float acc[NM][CB][NR];
 #pragma unroll
@@ -239,8 +242,8 @@ static int launch_gather(cbct_geom *g, AdjGeom &G, const float *sinoI, float *vo
     const int nq_total = g->d.n_views;
     G.nbase = g->d.n_views / NR;
     ViewChunk vc;
-    dim3 block(ADJ_BX, ADJ_BY);
-    dim3 grid((G.bx + ADJ_BX - 1) / ADJ_BX, (G.by + ADJ_BY - 1) / ADJ_BY, G.bz1 - G.bz0);
+    dim3 block(ADJ_BX, ADJ_BY, ADJ_BZ);
+    dim3 grid((G.bx + ADJ_BX - 1) / ADJ_BX, (G.by + ADJ_BY - 1) / ADJ_BY, (G.bz1 - G.bz0 + ADJ_BZ - 1) / ADJ_BZ);
     for (int q0 = 0; q0 < nq_total; q0 += CBCT_VIEWS_PER_LAUNCH) {
         int n = nq_total - q0;
         if (n > CBCT_VIEWS_PER_LAUNCH) n = CBCT_VIEWS_PER_LAUNCH;
