@@ -233,3 +233,41 @@ def fdk_frontend(g: Geom, proj) -> np.ndarray:
         for r in range(nv):
             out[i, r] = a * np.convolve(pt[i, r], h)[nu - 1:2 * nu - 1]
     return out
+
+
+def redundancy_weight(g: Geom) -> np.ndarray:
+    """Projection-domain redundancy weight w(u) for a laterally displaced detector ("FDK_w",
+    "P*(w y)": PAPER.md:167, :181, :186 name the weighting but give no formula -- reading R12,
+    DESIGN.md s.3: the smooth sine weighting of displaced-detector FDK, G. Wang, Med. Phys. 29 (2002)).
+    With the detector covering [u_min, u_max] (pixel CENTRES, mm, offset included) and
+    tau = min(|u_min|, |u_max|) the half-width of the band measured twice over a full turn:
+        w(u) = 1/2 (sin(pi atan(u/SDD) / (2 atan(tau/SDD))) + 1)   for |u| <= tau,
+        w(u) = 1 beyond tau on the long side (0 on the other side, which holds no pixels),
+    mirrored if the long side is the negative one; a centred detector (u_min = -u_max) gets
+    w = 1/2 everywhere.  Conjugate rays u and -u then always weigh w(u) + w(-u) = 1.  Returns w[nu]."""
+    nu = g.det_nu
+    u = (np.arange(nu) - 0.5 * (nu - 1)) * g.det_du_mm + g.det_off_u_mm
+    umin, umax = u[0], u[-1]
+    if abs(umin + umax) <= 1e-9 * max(abs(umin), abs(umax), 1.0) or umin * umax >= 0.0:
+        # centred detector: every ray is measured twice; a detector entirely on one side of the
+        # central ray has no doubly-measured band at all -- uniform weights in both cases
+        return np.full(nu, 0.5 if umin * umax < 0.0 or nu == 1 else 1.0)
+    sgn = 1.0 if umax > -umin else -1.0          # long side
+    tau = min(-umin, umax)
+    us = sgn * u
+    w = np.where(us > tau, 1.0, 0.0)
+    band = np.abs(us) <= tau
+    w[band] = 0.5 * (np.sin(np.pi * np.arctan(us[band] / g.sdd_mm) / (2.0 * np.arctan(tau / g.sdd_mm))) + 1.0)
+    return w
+
+
+def fdk_filter(g: Geom, proj, redundancy: bool = True) -> np.ndarray:
+    """Complete FDK front end (NEXT-1): q = dphi * fdk_frontend(w(u) * proj), dphi = 2 pi / n_views, so that
+    bp_fdk(q) IS the FDK_w reconstruction.  With redundancy=False, w = 1/2 (the textbook
+    dphi/2 of a centred detector, reading R11).  proj[C?, n_views, nv, nu]."""
+    proj = np.asarray(proj, dtype=np.float64)
+    w = redundancy_weight(g) if redundancy else np.full(g.det_nu, 0.5)
+    dphi = 2.0 * np.pi / g.n_views
+    if proj.ndim == 4:
+        return np.stack([dphi * fdk_frontend(g, p * w) for p in proj])
+    return dphi * fdk_frontend(g, proj * w)

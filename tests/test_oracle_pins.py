@@ -284,3 +284,50 @@ def test_tiny_sample_count(oracle_mod):
     n = o.count_samples(g)
     rays = 36 * 48 * 48
     assert 60.0 < n / rays < 75.0
+
+
+def test_p13_redundancy_weight_properties(oracle_mod):
+    """P13 (NEXT-1, reading R12): conjugate rays weigh w(u) + w(-u) = 1 inside the doubly measured band,
+    1 beyond it on the long side, continuous at the band edge, monotone; centred detector = 1/2;
+    a detector displaced the other way is the mirror image."""
+    o = oracle_mod
+    g, kw = G(o, det_nu=101, det_du_mm=2.0, det_off_u_mm=40.0)
+    w = o.redundancy_weight(g)
+    u = (np.arange(101) - 50) * 2.0 + 40.0        # -60 .. 140, tau = 60
+    assert w[0] == pytest.approx(0.0, abs=1e-15) and np.all(np.diff(w) >= -1e-15)
+    assert np.all(w[u > 60.0] == 1.0) and w[u == 60.0][0] == pytest.approx(1.0, abs=1e-15)
+    for k in range(1, 31):                         # u = +-2k are both pixel centres (u = 0 is pixel 30)
+        assert w[30 + k] + w[30 - k] == pytest.approx(1.0, abs=1e-14)
+    assert w[30] == pytest.approx(0.5, abs=1e-15)
+    # closed form at u = tau / 2
+    i = 30 + 15
+    want = 0.5 * (np.sin(np.pi * np.arctan(30.0 / 1536.0) / (2 * np.arctan(60.0 / 1536.0))) + 1.0)
+    assert w[i] == pytest.approx(want, abs=1e-15)
+    gm, _ = G(o, det_nu=101, det_du_mm=2.0, det_off_u_mm=-40.0)
+    assert np.allclose(o.redundancy_weight(gm), w[::-1], atol=1e-15)
+    gc, _ = G(o, det_nu=101, det_du_mm=2.0, det_off_u_mm=0.0)
+    assert np.all(o.redundancy_weight(gc) == 0.5)
+
+
+def test_p14_fdk_w_end_to_end_displaced_detector(oracle_mod):
+    """P14: with a displaced detector that truncates the ball's projection on the short side, FDK_w =
+    bp_fdk(fdk_filter(p, redundancy)) reproduces the ball's density in the mid-plane; without the
+    redundancy weight (uniform 1/2) it does not (the pin fails under a wrong / missing weight)."""
+    o = oracle_mod
+    nviews = 180
+    g, kw = G(o, n_views=nviews, det_nu=96, det_nv=48, det_du_mm=2.0, det_dv_mm=2.0, det_off_u_mm=50.0,
+              vol_nx=24, vol_ny=24, vol_nz=4)
+    ball = [(np.zeros(3), np.full(3, 40.0), np.eye(3), 0.02)]   # projects to |u| <= 61.5 mm; detector starts at -45
+    proj = an.ellipsoid_sinogram(kw, ball)
+    rec = o.bp_fdk(g, o.fdk_filter(g, proj, redundancy=True))[0]
+    ax = (np.arange(24) - 11.5) * 4.0
+    r = np.sqrt(ax[None, :] ** 2 + ax[:, None] ** 2)
+    mid = 0.5 * (rec[1] + rec[2])                  # z = -2 / +2 mm planes around the mid-plane
+    inside, outside = mid[r < 30.0], mid[r > 52.0]
+    assert abs(np.mean(inside) - 0.02) < 1e-4, np.mean(inside)
+    assert np.max(np.abs(inside - 0.02)) < 3e-4, np.max(np.abs(inside - 0.02))
+    # pre-convolution weighting is approximate away from the doubly measured band: a smooth
+    # background of ~9 % of the density remains outside the ball (independent of the view count)
+    assert np.max(np.abs(outside)) < 2.5e-3
+    bad = o.bp_fdk(g, o.fdk_filter(g, proj, redundancy=False))[0]
+    assert abs(np.mean(0.5 * (bad[1] + bad[2])[r < 30.0]) - 0.02) > 2e-3
