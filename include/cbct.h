@@ -115,6 +115,24 @@ int cbct_bp_adjoint(const cbct_geom *g, const float *sino, float *vol, int32_t c
  * weighted + ramp-filtered projection data; no dphi/2 factor is applied. */
 int cbct_bp_fdk(const cbct_geom *g, const float *sino, float *vol, int32_t channels, void *cuda_stream);
 
+/* NEXT-1: the projection-domain front end of FDK_w (ref [9] :397;
+ * readings R11, R12 in DESIGN.md s.3).  sino_out = dphi * a * ramp_u( w(u) * cos-weight * sino_in ), row by row,
+ * with a = du SID/SDD, Kak-Slaney taps h[0] = 1/(4a^2), h[odd n] = -1/(pi^2 n^2 a^2), h[even n] = 0, cos-weight
+ * SDD/sqrt(SDD^2+u^2+v^2) and dphi = 2 pi / n_views, so that cbct_bp_fdk(sino_out) is the reconstruction.
+ * flags & CBCT_FILTER_REDUNDANCY: w(u) = redundancy weight of a laterally displaced detector (smooth sine
+ * weighting; conjugate rays weigh 1 in total; see cbct_geom_redundancy_weights); otherwise w = 1/2.
+ * DEVICE pointers only, sino_out != sino_in, det_nu <= 2048; enqueued on `cuda_stream`. */
+#define CBCT_FILTER_REDUNDANCY 1
+int cbct_fdk_filter(const cbct_geom *g, const float *sino_in, float *sino_out, int32_t channels, int32_t flags,
+                    void *cuda_stream);
+
+/* sino_out = w(u) * sino_in, the weighting of P*(w y).  DEVICE pointers; in place allowed. */
+int cbct_redundancy_weight(const cbct_geom *g, const float *sino_in, float *sino_out, int32_t channels,
+                           void *cuda_stream);
+
+/* The det_nu redundancy weights w(u) in fp64 (host; needs no CUDA device). */
+int cbct_geom_redundancy_weights(const cbct_geom *g, double *w_out);
+
 /* Number of in-support samples of ONE channel: pairs (ray, k) with -1 < q < N
  * on every axis, counted analytically in fp64 on the host from the geometry
  * (the unit of the forward Gsamples/s metric).  Needs no CUDA device. */

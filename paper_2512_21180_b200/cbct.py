@@ -21,6 +21,7 @@ EXPORTS = (
     "cbct_geom_create", "cbct_geom_destroy", "cbct_fp", "cbct_bp_adjoint", "cbct_bp_fdk",
     "cbct_geom_count_samples", "cbct_geom_num_slabs", "cbct_geom_launch_count",
     "cbct_geom_profile", "cbct_geom_profile_read",
+    "cbct_fdk_filter", "cbct_redundancy_weight", "cbct_geom_redundancy_weights",
     "cbct_status_string", "cbct_last_cuda_error",
 )
 
@@ -70,6 +71,9 @@ def load_library() -> ctypes.CDLL:
     L.cbct_geom_profile.argtypes = [vp, ctypes.c_int]
     L.cbct_geom_profile_read.argtypes = [vp, ctypes.c_int, ctypes.POINTER(ctypes.c_double),
                                          ctypes.POINTER(ctypes.c_uint64)]
+    L.cbct_fdk_filter.argtypes = [vp, vp, vp, i32, i32, vp]
+    L.cbct_redundancy_weight.argtypes = [vp, vp, vp, i32, vp]
+    L.cbct_geom_redundancy_weights.argtypes = [vp, ctypes.POINTER(ctypes.c_double)]
     L.cbct_status_string.argtypes = [ctypes.c_int]
     L.cbct_status_string.restype = ctypes.c_char_p
     L.cbct_last_cuda_error.restype = ctypes.c_char_p
@@ -171,6 +175,26 @@ class Geometry:
         ps, pv = _ptr_and_keep(sino, channels * self.n_sino), _ptr_and_keep(vol, channels * self.n_vol)
         _check(load_library().cbct_bp_fdk(self._h, ps, pv, channels, _stream_handle(stream)))
         return vol
+
+    # --- NEXT-1: FDK front end ------------------------------------------------
+    def fdk_filter(self, sino_in, sino_out, channels: int = 1, redundancy: bool = True, stream=None):
+        """cbct_fdk_filter: weighted + ramp-filtered projections q such that bp_fdk(q) = FDK_w."""
+        pi, po = _ptr_and_keep(sino_in, channels * self.n_sino), _ptr_and_keep(sino_out, channels * self.n_sino)
+        _check(load_library().cbct_fdk_filter(self._h, pi, po, channels, 1 if redundancy else 0,
+                                              _stream_handle(stream)))
+        return sino_out
+
+    def redundancy_weight(self, sino_in, sino_out, channels: int = 1, stream=None):
+        """cbct_redundancy_weight: sino_out = w(u) * sino_in (in place allowed)."""
+        pi, po = _ptr_and_keep(sino_in, channels * self.n_sino), _ptr_and_keep(sino_out, channels * self.n_sino)
+        _check(load_library().cbct_redundancy_weight(self._h, pi, po, channels, _stream_handle(stream)))
+        return sino_out
+
+    def redundancy_weights(self) -> np.ndarray:
+        w = np.empty(self.desc.det_nu, dtype=np.float64)
+        _check(load_library().cbct_geom_redundancy_weights(
+            self._h, w.ctypes.data_as(ctypes.POINTER(ctypes.c_double))))
+        return w
 
     # --- host-side queries --------------------------------------------------
     def count_samples(self) -> int:

@@ -104,11 +104,12 @@ static void prof_clear(cbct_geom *g);
 extern "C" int cbct_geom_destroy(cbct_geom *g)
 {
     if (!g) return CBCT_ERR_INVALID_ARG;
-    if (g->ws_vol || g->ws_sino || g->ws_sino2 || g->ws_stage || g->copy_stream) {
+    if (g->ws_vol || g->ws_sino || g->ws_sino2 || g->ws_stage || g->copy_stream || g->d_filter_tab) {
         cudaDeviceSynchronize();
         cudaFree(g->ws_vol);
         cudaFree(g->ws_sino);
         cudaFree(g->ws_sino2);
+        cudaFree(g->d_filter_tab);
         cudaFree(g->ws_stage);
         for (int i = 0; i < 4; ++i)
             if (g->ev[i]) cudaEventDestroy(g->ev[i]);

@@ -65,6 +65,7 @@ struct cbct_geom {
     cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
     uint64_t launches = 0;
     int64_t sample_count = -1;
+    float *d_filter_tab = nullptr;  // FDK front-end tables (cbct_fdk_filter.cu), built on first use
     // optional per-launch event pairs of the three main kernels (cbct_geom_profile)
     bool profiling = false;
     std::vector<std::pair<cudaEvent_t, cudaEvent_t>> prof[3];

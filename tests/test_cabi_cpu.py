@@ -101,3 +101,13 @@ def test_missing_library_is_loud(cbct, monkeypatch, tmp_path):
     monkeypatch.setattr(cbct, "LIB_PATH", str(tmp_path / "nope.so"))
     with pytest.raises(cbct.CbctError, match="missing"):
         cbct.load_library()
+
+
+@pytest.mark.parametrize("over", [dict(), dict(det_off_u_mm=115.0, det_nu=128, det_du_mm=1.6),
+                                  dict(det_off_u_mm=-37.3, det_nu=77), dict(det_off_u_mm=400.0)])
+def test_redundancy_weights_match_oracle(cbct, oracle_mod, over):
+    """NEXT-1: the library's host table of w(u) (reading R12) equals the oracle's."""
+    kw = dict(synth.geom_kwargs(synth.CONFIGS["tiny"]))
+    kw.update(over)
+    w = cbct.Geometry(**kw).redundancy_weights()
+    assert np.max(np.abs(w - oracle_mod.redundancy_weight(oracle_mod.Geom(**kw)))) <= 1e-15
