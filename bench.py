@@ -205,6 +205,26 @@ def main():
     t_total = evs[0][0].elapsed_time(evs[-1][3]) / args.steps
     t_fp, t_adj, t_fdk, t_total = cdist.max_over_ranks([t_fp, t_adj, t_fdk, t_total], device="cuda")
 
+    # NEXT-1 kernels (not part of the step): FDK front end and redundancy weighting over all channels
+    next1 = None
+    if not streamed:
+        evn = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
+        g.fdk_filter(sino_in, sino_out, C)
+        cdist.barrier(cuda=True)
+        evn[0].record()
+        for _ in range(3):
+            g.fdk_filter(sino_in, sino_out, C)
+        evn[1].record()
+        for _ in range(3):
+            g.redundancy_weight(sino_in, sino_out, C)
+        evn[2].record()
+        cdist.barrier(cuda=True)
+        t_flt, t_w = evn[0].elapsed_time(evn[1]) / 3, evn[1].elapsed_time(evn[2]) / 3
+        next1 = {"fdk_filter_ms": t_flt, "redundancy_weight_ms": t_w,
+                 "redundancy_weight_hbm_gbs": 2 * sino_h.nbytes / (t_w * 1e-3) / 1e9,
+                 "fdk_filter_gmacs": C * cfg["n_views"] * cfg["det_nv"] * cfg["det_nu"] * (cfg["det_nu"] // 2 + 1)
+                 / (t_flt * 1e-3) / 1e9}
+
     # end to end through the C ABI with HOST (pinned) buffers: copies inside the timed region
     e2e = None
     if not args.no_e2e and not streamed:
@@ -297,6 +317,8 @@ def main():
             "call_ms": {"cbct_fp": t_fp, "cbct_bp_adjoint": t_adj, "cbct_bp_fdk": t_fdk},
             "samples_per_channel": n_samples, "voxel_views_per_channel": n_vv,
             "gpu_launches": int(launches), "clocks": clocks, "roofline": roofline}
+    if next1:
+        line["next1"] = next1
     if e2e:
         line["e2e"] = e2e
     if not args.no_cpu_baseline and world == 1:
