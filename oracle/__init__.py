@@ -271,3 +271,57 @@ def fdk_filter(g: Geom, proj, redundancy: bool = True) -> np.ndarray:
     if proj.ndim == 4:
         return np.stack([dphi * fdk_frontend(g, p * w) for p in proj])
     return dphi * fdk_frontend(g, proj * w)
+
+
+# ---------------------------------------------------------------------------
+# NEXT-2: field-of-view tensor and the resampling operators of the multiscale scheme
+# ---------------------------------------------------------------------------
+def fov(g: Geom) -> np.ndarray:
+    """V(p) = (number of projections where voxel p is visible) / (total projection count).
+    Reading R21 (DESIGN.md s.3): voxel p is visible in view i when its CENTRE projects onto the panel's
+    active area, -1/2 <= fu < nu - 1/2 and -1/2 <= fv < nv - 1/2 in pixel-index coordinates (the union of the
+    pixel footprints), with (fu, fv) as in the FDK backprojection (R9).  Returns V[nz, ny, nx] fp64."""
+    x = g.vol_cx_mm + (np.arange(g.vol_nx) - 0.5 * (g.vol_nx - 1)) * g.vox_mm
+    y = g.vol_cy_mm + (np.arange(g.vol_ny) - 0.5 * (g.vol_ny - 1)) * g.vox_mm
+    z = g.vol_cz_mm + (np.arange(g.vol_nz) - 0.5 * (g.vol_nz - 1)) * g.vox_mm
+    X, Y, Z = x[None, None, :], y[None, :, None], z[:, None, None]
+    count = np.zeros((g.vol_nz, g.vol_ny, g.vol_nx), dtype=np.int64)
+    angles = g.angles_rad if g.angles_rad is not None else [2.0 * np.pi * i / g.n_views for i in range(g.n_views)]
+    for phi in angles:
+        c, s = np.cos(phi), np.sin(phi)
+        U = g.sid_mm - (X * c + Y * s)
+        ustar = g.sdd_mm * (-X * s + Y * c) / U
+        vstar = g.sdd_mm * Z / U
+        fu = (ustar - g.det_off_u_mm) / g.det_du_mm + 0.5 * (g.det_nu - 1)
+        fv = (vstar - g.det_off_v_mm) / g.det_dv_mm + 0.5 * (g.det_nv - 1)
+        count += ((fu >= -0.5) & (fu < g.det_nu - 0.5) & (fv >= -0.5) & (fv < g.det_nv - 0.5))
+    return count / float(g.n_views)
+
+
+def downsample(z, factor: int) -> np.ndarray:
+    """Downsample_alpha: average pooling of the last three axes by `factor` = 1/alpha
+    (sizes must be multiples of factor).  z[..., nz, ny, nx] -> [..., nz/f, ny/f, nx/f]."""
+    z = np.asarray(z, dtype=np.float64)
+    f = factor
+    nz, ny, nx = z.shape[-3:]
+    assert nz % f == 0 and ny % f == 0 and nx % f == 0
+    return z.reshape(z.shape[:-3] + (nz // f, f, ny // f, f, nx // f, f)).mean(axis=(-5, -3, -1))
+
+
+def upsample(z, factor: int) -> np.ndarray:
+    """Upsample ("nearest upsampling"): every voxel repeated `factor` times along the last
+    three axes."""
+    z = np.asarray(z, dtype=np.float64)
+    for ax in (-3, -2, -1):
+        z = np.repeat(z, factor, axis=ax)
+    return z
+
+
+def proj_down(p, factor: int) -> np.ndarray:
+    """ProjDown_alpha: keeps every `factor`-th projection (views 0, f, 2f, ...; reading R14) and
+    average-pools each kept projection by `factor` along both detector axes.  p[..., n_views, nv, nu]."""
+    p = np.asarray(p, dtype=np.float64)[..., ::factor, :, :]
+    f = factor
+    nv, nu = p.shape[-2:]
+    assert nv % f == 0 and nu % f == 0
+    return p.reshape(p.shape[:-2] + (nv // f, f, nu // f, f)).mean(axis=(-3, -1))

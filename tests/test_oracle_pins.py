@@ -331,3 +331,46 @@ def test_p14_fdk_w_end_to_end_displaced_detector(oracle_mod):
     assert np.max(np.abs(outside)) < 2.5e-3
     bad = o.bp_fdk(g, o.fdk_filter(g, proj, redundancy=False))[0]
     assert abs(np.mean(0.5 * (bad[1] + bad[2])[r < 30.0]) - 0.02) > 2e-3
+
+
+def test_p15_fov_closed_forms(oracle_mod):
+    """P15 (NEXT-2): V = 1 under a detector that sees everything; for a half-fan detector a mid-plane voxel
+    at radius r beyond the short side's field of view is visible for the fraction 1/2 + asin(kappa)/pi of a
+    turn, kappa = |u_lo| SID / (r sqrt(SDD^2 + u_lo^2)), u_lo the panel's short edge (from
+    SDD r sin(psi) >= u_lo (SID - r cos(psi))); inside that radius it is always visible."""
+    o = oracle_mod
+    gbig, _ = G(o, det_nu=400, det_nv=400, n_views=12)
+    assert np.all(o.fov(gbig) == 1.0)
+    n_views = 720
+    g, kw = G(o, n_views=n_views, det_nu=128, det_nv=256, det_du_mm=1.6, det_dv_mm=1.6, det_off_u_mm=60.0,
+              vol_nx=33, vol_ny=33, vol_nz=1, vox_mm=4.0)
+    V = o.fov(g)[0]
+    u_lo = -0.5 * 128 * 1.6 + 60.0          # panel edge (half a pixel beyond the first pixel centre)
+    ax = (np.arange(33) - 16) * 4.0
+    r = np.sqrt(ax[None, :] ** 2 + ax[:, None] ** 2)
+    r_short = 1000.0 * abs(u_lo) / np.sqrt(1536.0 ** 2 + u_lo ** 2)
+    assert np.all(V[r < r_short - 1.0] == 1.0)
+    sel = (r > r_short + 1.0)
+    kappa = abs(u_lo) * 1000.0 / (r[sel] * np.sqrt(1536.0 ** 2 + u_lo ** 2))
+    want = 0.5 + np.arcsin(kappa) / np.pi
+    assert np.max(np.abs(V[sel] - want)) <= 2.0 / n_views
+    assert V.min() > 0.5
+
+
+def test_p16_resampling_definitions(oracle_mod):
+    """P16 (NEXT-2): average pooling preserves means and constants, is linear, and inverts nearest upsampling;
+    ProjDown keeps views 0, f, 2f, ... and pools the detector; a hand-computed 2x2x2 block."""
+    o = oracle_mod
+    rng = np.random.default_rng(3)
+    z = rng.random((2, 8, 12, 4))
+    d2 = o.downsample(z, 2)
+    assert d2.shape == (2, 4, 6, 2) and np.allclose(d2.mean(), z.mean())
+    assert d2[1, 2, 3, 1] == pytest.approx(z[1, 4:6, 6:8, 2:4].sum() / 8.0, abs=1e-15)
+    assert np.allclose(o.downsample(o.upsample(d2, 2), 2), d2, atol=1e-15)
+    up = o.upsample(d2, 4)
+    assert up.shape == (2, 16, 24, 8) and np.all(up[0, 5, 9, 3] == d2[0, 1, 2, 0])
+    assert np.allclose(o.downsample(z, 4), o.downsample(d2, 2), atol=1e-15)
+    p = rng.random((3, 8, 4, 6))
+    pd = o.proj_down(p, 2)
+    assert pd.shape == (3, 4, 2, 3)
+    assert pd[2, 1, 1, 2] == pytest.approx(p[2, 2, 2:4, 4:6].sum() / 4.0, abs=1e-15)
