@@ -133,6 +133,23 @@ int cbct_redundancy_weight(const cbct_geom *g, const float *sino_in, float *sino
 /* The det_nu redundancy weights w(u) in fp64 (host; needs no CUDA device). */
 int cbct_geom_redundancy_weights(const cbct_geom *g, double *w_out);
 
+/* NEXT-2.  Field-of-view tensor: vol_out[z,y,x] = (number of views in which the
+ * centre of voxel (z,y,x) projects onto the panel's active area, -1/2 <= fu < nu-1/2 and -1/2 <= fv < nv-1/2) /
+ * n_views (reading R21).  vol_out: nz*ny*nx floats, DEVICE pointer, overwritten. */
+int cbct_fov(const cbct_geom *g, float *vol_out, void *cuda_stream);
+
+/* Resampling operators of the multiscale scheme; plain arrays, DEVICE pointers, `n_outer` leading
+ * items (channels).  cbct_downsample: average pooling by `factor` of in[n_outer][nz_in][ny_in][nx_in] (sizes must be
+ * multiples of factor).  cbct_upsample: nearest upsampling, out[n_outer][nz_in f][ny_in f][nx_in f].
+ * cbct_proj_down: keeps views 0, f, 2f, ... of in[n_outer][n_views_in][nv_in][nu_in] and average-pools the detector
+ * by f: out[n_outer][ceil(n_views_in / f)][nv_in / f][nu_in / f]. */
+int cbct_downsample(const float *in, float *out, int64_t n_outer, int32_t nz_in, int32_t ny_in, int32_t nx_in,
+                    int32_t factor, void *cuda_stream);
+int cbct_upsample(const float *in, float *out, int64_t n_outer, int32_t nz_in, int32_t ny_in, int32_t nx_in,
+                  int32_t factor, void *cuda_stream);
+int cbct_proj_down(const float *in, float *out, int64_t n_outer, int32_t n_views_in, int32_t nv_in, int32_t nu_in,
+                   int32_t factor, void *cuda_stream);
+
 /* Number of in-support samples of ONE channel: pairs (ray, k) with -1 < q < N
  * on every axis, counted analytically in fp64 on the host from the geometry
  * (the unit of the forward Gsamples/s metric).  Needs no CUDA device. */

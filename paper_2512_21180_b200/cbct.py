@@ -22,6 +22,7 @@ EXPORTS = (
     "cbct_geom_count_samples", "cbct_geom_num_slabs", "cbct_geom_launch_count",
     "cbct_geom_profile", "cbct_geom_profile_read",
     "cbct_fdk_filter", "cbct_redundancy_weight", "cbct_geom_redundancy_weights",
+    "cbct_fov", "cbct_downsample", "cbct_upsample", "cbct_proj_down",
     "cbct_status_string", "cbct_last_cuda_error",
 )
 
@@ -74,6 +75,11 @@ def load_library() -> ctypes.CDLL:
     L.cbct_fdk_filter.argtypes = [vp, vp, vp, i32, i32, vp]
     L.cbct_redundancy_weight.argtypes = [vp, vp, vp, i32, vp]
     L.cbct_geom_redundancy_weights.argtypes = [vp, ctypes.POINTER(ctypes.c_double)]
+    L.cbct_fov.argtypes = [vp, vp, vp]
+    i64 = ctypes.c_int64
+    L.cbct_downsample.argtypes = [vp, vp, i64, i32, i32, i32, i32, vp]
+    L.cbct_upsample.argtypes = [vp, vp, i64, i32, i32, i32, i32, vp]
+    L.cbct_proj_down.argtypes = [vp, vp, i64, i32, i32, i32, i32, vp]
     L.cbct_status_string.argtypes = [ctypes.c_int]
     L.cbct_status_string.restype = ctypes.c_char_p
     L.cbct_last_cuda_error.restype = ctypes.c_char_p
@@ -196,6 +202,12 @@ class Geometry:
             self._h, w.ctypes.data_as(ctypes.POINTER(ctypes.c_double))))
         return w
 
+    # --- NEXT-2: field-of-view tensor -----------------------------------------
+    def fov(self, vol_out, stream=None):
+        """cbct_fov: V[nz,ny,nx] = fraction of views in which each voxel is visible."""
+        _check(load_library().cbct_fov(self._h, _ptr_and_keep(vol_out, self.n_vol), _stream_handle(stream)))
+        return vol_out
+
     # --- host-side queries --------------------------------------------------
     def count_samples(self) -> int:
         out = ctypes.c_uint64()
@@ -221,3 +233,39 @@ class Geometry:
         out = ctypes.c_uint64()
         _check(load_library().cbct_geom_launch_count(self._h, ctypes.byref(out)))
         return int(out.value)
+
+
+# --- NEXT-2: resampling operators of the multiscale scheme (plain arrays, no geometry) ---
+def _shape4(t):
+    shp = tuple(t.shape)
+    if len(shp) < 3:
+        raise CbctError("expected at least 3 dimensions")
+    outer = int(np.prod(shp[:-3])) if len(shp) > 3 else 1
+    return outer, shp[-3], shp[-2], shp[-1]
+
+
+def downsample(vol_in, vol_out, factor: int, stream=None):
+    """cbct_downsample: average pooling of the last three axes by `factor`."""
+    o, nz, ny, nx = _shape4(vol_in)
+    pi = _ptr_and_keep(vol_in, o * nz * ny * nx)
+    po = _ptr_and_keep(vol_out, o * (nz // factor) * (ny // factor) * (nx // factor))
+    _check(load_library().cbct_downsample(pi, po, o, nz, ny, nx, factor, _stream_handle(stream)))
+    return vol_out
+
+
+def upsample(vol_in, vol_out, factor: int, stream=None):
+    """cbct_upsample: nearest upsampling of the last three axes by `factor`."""
+    o, nz, ny, nx = _shape4(vol_in)
+    pi = _ptr_and_keep(vol_in, o * nz * ny * nx)
+    po = _ptr_and_keep(vol_out, o * nz * ny * nx * factor ** 3)
+    _check(load_library().cbct_upsample(pi, po, o, nz, ny, nx, factor, _stream_handle(stream)))
+    return vol_out
+
+
+def proj_down(sino_in, sino_out, factor: int, stream=None):
+    """cbct_proj_down: keep every `factor`-th view, average-pool the detector by `factor`."""
+    o, nviews, nv, nu = _shape4(sino_in)
+    pi = _ptr_and_keep(sino_in, o * nviews * nv * nu)
+    po = _ptr_and_keep(sino_out, o * (-(-nviews // factor)) * (nv // factor) * (nu // factor))
+    _check(load_library().cbct_proj_down(pi, po, o, nviews, nv, nu, factor, _stream_handle(stream)))
+    return sino_out

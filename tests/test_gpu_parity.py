@@ -441,3 +441,41 @@ def test_next1_fdk_w_end_to_end(cbct, oracle_mod):
     r = np.sqrt(ax[None, :] ** 2 + ax[:, None] ** 2)
     mid = 0.5 * (rec[1] + rec[2])
     assert abs(np.mean(mid[r < 30.0]) - 0.02) < 1e-4
+
+
+@pytest.mark.parametrize("over", [dict(), dict(det_off_u_mm=40.0, det_nu=40, det_nv=30, n_views=50),
+                                  dict(vol_nx=37, vol_ny=29, vol_nz=21, vol_cx_mm=5.0, det_off_v_mm=-7.0, n_views=11),
+                                  dict(n_views=1040, vol_nx=16, vol_ny=16, vol_nz=6, det_nu=24, det_nv=12, det_off_u_mm=20.0)])
+def test_next2_fov(cbct, oracle_mod, over):
+    """NEXT-2: the field-of-view tensor V equals the oracle's view counts exactly (integer decision in fp64)."""
+    kw = dict(synth.geom_kwargs(synth.CONFIGS["tiny"]))
+    kw.update(over)
+    g = cbct.Geometry(**kw)
+    out = torch.full(g.vol_shape, float("nan"), device="cuda")
+    g.fov(out)
+    torch.cuda.synchronize()
+    want = oracle_mod.fov(oracle_mod.Geom(**kw))
+    got = out.cpu().numpy().astype(np.float64)
+    assert np.array_equal(np.rint(got * kw["n_views"]), np.rint(want * kw["n_views"]))
+    assert np.max(np.abs(got - want)) <= 1e-6
+
+
+def test_next2_resampling(cbct, oracle_mod):
+    """NEXT-2: Downsample (average pooling), Upsample (nearest), ProjDown against the oracle."""
+    rng = np.random.default_rng(23)
+    z = rng.standard_normal((3, 8, 12, 20)).astype(np.float32)
+    for f in (2, 4):
+        out = torch.empty((3, 8 // f, 12 // f, 20 // f), device="cuda")
+        cbct.downsample(dev(z), out, f)
+        want = oracle_mod.downsample(z.astype(np.float64), f)
+        assert np.max(np.abs(out.cpu().numpy() - want)) <= 1e-6
+        up = torch.empty((3, 8 * f, 12 * f, 20 * f), device="cuda")
+        cbct.upsample(dev(z), up, f)
+        assert np.array_equal(up.cpu().numpy(), oracle_mod.upsample(z, f).astype(np.float32))
+    p = rng.random((2, 9, 8, 12)).astype(np.float32)
+    for f in (2, 4):
+        out = torch.empty((2, -(-9 // f), 8 // f, 12 // f), device="cuda")
+        cbct.proj_down(dev(p), out, f)
+        assert np.max(np.abs(out.cpu().numpy() - oracle_mod.proj_down(p.astype(np.float64), f))) <= 1e-6
+    with pytest.raises(cbct.CbctError):
+        cbct.downsample(dev(z), torch.empty((3, 2, 4, 6), device="cuda"), 3)
