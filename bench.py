@@ -224,6 +224,28 @@ def main():
                  "redundancy_weight_hbm_gbs": 2 * sino_h.nbytes / (t_w * 1e-3) / 1e9,
                  "fdk_filter_gmacs": C * cfg["n_views"] * cfg["det_nv"] * cfg["det_nu"] * (cfg["det_nu"] // 2 + 1)
                  / (t_flt * 1e-3) / 1e9}
+        # NEXT-2: FoV tensor and the resampling operators (streaming kernels: bytes moved / time)
+        def timed(fn, reps=3):
+            fn()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            torch.cuda.synchronize()
+            a.record()
+            for _ in range(reps):
+                fn()
+            b.record()
+            torch.cuda.synchronize()
+            return a.elapsed_time(b) / reps
+        n = cfg["vol_nx"]
+        half = torch.empty((C, n // 2, n // 2, n // 2), device="cuda")
+        pd = torch.empty((C, cfg["n_views"] // 2, cfg["det_nv"] // 2, cfg["det_nu"] // 2), device="cuda")
+        t_fov = timed(lambda: g.fov(vol_out[0]))
+        t_dn = timed(lambda: cbct.downsample(vol, half, 2))
+        t_up = timed(lambda: cbct.upsample(half, vol_out, 2))
+        t_pd = timed(lambda: cbct.proj_down(sino_in, pd, 2))
+        next1.update({"fov_ms": t_fov, "fov_gvoxel_views_per_s": n_vv / (t_fov * 1e-3) / 1e9,
+                      "downsample2_ms": t_dn, "downsample2_hbm_gbs": (vol_h.nbytes * 1.125) / (t_dn * 1e-3) / 1e9,
+                      "upsample2_ms": t_up, "upsample2_hbm_gbs": (vol_h.nbytes * 1.125) / (t_up * 1e-3) / 1e9,
+                      "proj_down2_ms": t_pd, "proj_down2_hbm_gbs": (sino_h.nbytes * 0.5 * 1.25) / (t_pd * 1e-3) / 1e9})
 
     # end to end through the C ABI with HOST (pinned) buffers: copies inside the timed region
     e2e = None
@@ -318,7 +340,7 @@ def main():
             "samples_per_channel": n_samples, "voxel_views_per_channel": n_vv,
             "gpu_launches": int(launches), "clocks": clocks, "roofline": roofline}
     if next1:
-        line["next1"] = next1
+        line["next"] = next1
     if e2e:
         line["e2e"] = e2e
     if not args.no_cpu_baseline and world == 1:

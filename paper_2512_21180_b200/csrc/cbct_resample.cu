@@ -69,69 +69,104 @@ extern "C" int cbct_fov(const cbct_geom *gc, float *vol_out, void *stream)
 // ---------------------------------------------------------------------------
 // resampling (no geometry handle: plain array operators)
 // ---------------------------------------------------------------------------
+// Row-oriented streaming kernels: a CTA of 64 x 4 threads takes 4 output rows at a time (grid-stride over
+// rows, so the only integer divisions are per row), threads run along x with vector loads / stores so that
+// every 32-byte sector moved is fully used.  F = pooling factor (2 and 4 vectorised; 0 = any factor, scalar).
+template <int F> struct VecOf { typedef float type; };
+template <> struct VecOf<2> { typedef float2 type; };
+template <> struct VecOf<4> { typedef float4 type; };
+__device__ __forceinline__ float hsum(float v) { return v; }
+__device__ __forceinline__ float hsum(float2 v) { return v.x + v.y; }
+__device__ __forceinline__ float hsum(float4 v) { return (v.x + v.y) + (v.z + v.w); }
+
+// sum over an F-wide run of `rows` input rows spaced `pitch` floats apart, starting at p
+template <int F>
+__device__ __forceinline__ float pool_rows(const float *__restrict__ p, int f, size_t pitch, int rows)
+{
+    float acc = 0.f;
+    if (F == 0) {
+        for (int j = 0; j < rows; ++j)
+            for (int i = 0; i < f; ++i) acc += __ldg(p + j * pitch + i);
+    } else {
+        typedef typename VecOf<F>::type V;
+#pragma unroll
+        for (int j = 0; j < F; ++j) acc += hsum(__ldg(reinterpret_cast<const V *>(p + j * pitch)));
+    }
+    return acc;
+}
+
 // out[o][z][y][x] = mean of the f^3 block of in[o] (in dims: nz f, ny f, nx f)
+template <int F>
 __global__ void __launch_bounds__(256)
-downsample_kernel(const float *__restrict__ in, float *__restrict__ out, size_t n_out, int nz, int ny, int nx, int f)
+downsample_kernel(const float *__restrict__ in, float *__restrict__ out, size_t n_rows, int nz, int ny, int nx, int f)
 {
     const float inv = 1.0f / (float)(f * f * f);
-    for (size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x; e < n_out; e += (size_t)gridDim.x * blockDim.x) {
-        const int x = (int)(e % nx);
-        size_t t = e / nx;
-        const int y = (int)(t % ny);
-        t /= ny;
-        const int z = (int)(t % nz);
-        const size_t o = t / nz;
-        const float *p = in + (((o * nz + z) * f) * (size_t)(ny * f) + (size_t)y * f) * (size_t)(nx * f) + (size_t)x * f;
-        float acc = 0.f;
-        for (int k = 0; k < f; ++k)
-            for (int j = 0; j < f; ++j)
-                for (int i = 0; i < f; ++i) acc += __ldg(p + ((size_t)k * (ny * f) + j) * (size_t)(nx * f) + i);
-        out[e] = acc * inv;
+    const size_t in_pitch = (size_t)nx * f, in_plane = in_pitch * ny * f;
+    for (size_t r = (size_t)blockIdx.x * blockDim.y + threadIdx.y; r < n_rows; r += (size_t)gridDim.x * blockDim.y) {
+        const int y = (int)(r % ny);
+        const size_t oz = r / ny;  // o * nz + z
+        const float *src = in + (oz * f) * in_plane + (size_t)y * f * in_pitch;
+        for (int x = threadIdx.x; x < nx; x += blockDim.x) {
+            float acc = 0.f;
+            for (int k = 0; k < f; ++k) acc += pool_rows<F>(src + k * in_plane + (size_t)x * f, f, in_pitch, f);
+            out[r * nx + x] = acc * inv;
+        }
     }
 }
 
-// out[o][z][y][x] = in[o][z / f][y / f][x / f]   (out dims: nz f, ny f, nx f)
+// out[o][z][y][x] = in[o][z / f][y / f][x / f]   (out dims: nz f, ny f, nx f).  A thread expands its piece of one
+// INPUT row into the f x f output rows it feeds (4 outputs per store when the row length allows).
 __global__ void __launch_bounds__(256)
-upsample_kernel(const float *__restrict__ in, float *__restrict__ out, size_t n_out, int nz, int ny, int nx, int f)
+upsample_kernel(const float *__restrict__ in, float *__restrict__ out, size_t n_rows, int nz, int ny, int nx, int f,
+                int vec4)
 {
-    const int NX = nx * f, NY = ny * f, NZ = nz * f;
-    for (size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x; e < n_out; e += (size_t)gridDim.x * blockDim.x) {
-        const int x = (int)(e % NX);
-        size_t t = e / NX;
-        const int y = (int)(t % NY);
-        t /= NY;
-        const int z = (int)(t % NZ);
-        const size_t o = t / NZ;
-        out[e] = __ldg(in + ((o * nz + z / f) * ny + y / f) * (size_t)nx + x / f);
+    const int NX = nx * f;
+    const size_t out_pitch = (size_t)NX, out_plane = out_pitch * ny * f;
+    for (size_t r = (size_t)blockIdx.x * blockDim.y + threadIdx.y; r < n_rows; r += (size_t)gridDim.x * blockDim.y) {
+        const int y = (int)(r % ny);
+        const size_t oz = r / ny;  // o * nz + z
+        const float *src = in + r * nx;
+        float *dst = out + (oz * f) * out_plane + (size_t)y * f * out_pitch;
+        if (vec4) {
+            for (int x = threadIdx.x * 4; x < NX; x += blockDim.x * 4) {
+                const float4 v = make_float4(__ldg(src + x / f), __ldg(src + (x + 1) / f), __ldg(src + (x + 2) / f),
+                                             __ldg(src + (x + 3) / f));
+                for (int k = 0; k < f; ++k)
+                    for (int j = 0; j < f; ++j) *reinterpret_cast<float4 *>(dst + k * out_plane + j * out_pitch + x) = v;
+            }
+        } else {
+            for (int x = threadIdx.x; x < NX; x += blockDim.x) {
+                const float v = __ldg(src + x / f);
+                for (int k = 0; k < f; ++k)
+                    for (int j = 0; j < f; ++j) dst[k * out_plane + j * out_pitch + x] = v;
+            }
+        }
     }
 }
 
-// out[o][i][v][u] = mean of the f^2 block of in[o][i f] (in dims: n_views f', nv f, nu f; views i f kept)
+// out[o][i][v][u] = mean of the f^2 block of in[o][i f] (in dims: n_views_in, nv f, nu f; views i f kept)
+template <int F>
 __global__ void __launch_bounds__(256)
-proj_down_kernel(const float *__restrict__ in, float *__restrict__ out, size_t n_out, int n_views_in, int n_views_out,
+proj_down_kernel(const float *__restrict__ in, float *__restrict__ out, size_t n_rows, int n_views_in, int n_views_out,
                  int nv, int nu, int f)
 {
     const float inv = 1.0f / (float)(f * f);
-    for (size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x; e < n_out; e += (size_t)gridDim.x * blockDim.x) {
-        const int u = (int)(e % nu);
-        size_t t = e / nu;
-        const int v = (int)(t % nv);
-        t /= nv;
-        const int i = (int)(t % n_views_out);
-        const size_t o = t / n_views_out;
-        const float *p = in + ((o * n_views_in + (size_t)i * f) * (size_t)(nv * f) + (size_t)v * f) * (size_t)(nu * f) +
-                         (size_t)u * f;
-        float acc = 0.f;
-        for (int j = 0; j < f; ++j)
-            for (int k = 0; k < f; ++k) acc += __ldg(p + (size_t)j * (nu * f) + k);
-        out[e] = acc * inv;
+    const size_t in_pitch = (size_t)nu * f, in_img = in_pitch * nv * f;
+    for (size_t r = (size_t)blockIdx.x * blockDim.y + threadIdx.y; r < n_rows; r += (size_t)gridDim.x * blockDim.y) {
+        const int v = (int)(r % nv);
+        const size_t oi = r / nv;
+        const int i = (int)(oi % n_views_out);
+        const size_t o = oi / n_views_out;
+        const float *src = in + (o * n_views_in + (size_t)i * f) * in_img + (size_t)v * f * in_pitch;
+        for (int u = threadIdx.x; u < nu; u += blockDim.x)
+            out[r * nu + u] = pool_rows<F>(src + (size_t)u * f, f, in_pitch, f) * inv;
     }
 }
 
-static unsigned blocks_for(size_t n)
+static unsigned row_blocks(size_t rows)
 {
-    size_t b = (n + 255) / 256;
-    return (unsigned)(b < 148u * 16u ? (b ? b : 1) : 148u * 16u);
+    size_t b = (rows + 3) / 4;
+    return (unsigned)(b < 148u * 32u ? (b ? b : 1) : 148u * 32u);
 }
 
 static int finish(const char *what)
@@ -147,8 +182,12 @@ extern "C" int cbct_downsample(const float *in, float *out, int64_t n_outer, int
     if (!in || !out || n_outer < 1 || factor < 1 || nz_in < 1 || ny_in < 1 || nx_in < 1) return CBCT_ERR_INVALID_ARG;
     if (nz_in % factor || ny_in % factor || nx_in % factor) return CBCT_ERR_INVALID_ARG;
     const int nz = nz_in / factor, ny = ny_in / factor, nx = nx_in / factor;
-    const size_t n = (size_t)n_outer * nz * ny * nx;
-    downsample_kernel<<<blocks_for(n), 256, 0, (cudaStream_t)stream>>>(in, out, n, nz, ny, nx, factor);
+    const size_t rows = (size_t)n_outer * nz * ny;
+    const bool al = ((uintptr_t)in % 16 == 0);
+    const dim3 block(64, 4);
+    if (factor == 2 && al) downsample_kernel<2><<<row_blocks(rows), block, 0, (cudaStream_t)stream>>>(in, out, rows, nz, ny, nx, 2);
+    else if (factor == 4 && al) downsample_kernel<4><<<row_blocks(rows), block, 0, (cudaStream_t)stream>>>(in, out, rows, nz, ny, nx, 4);
+    else downsample_kernel<0><<<row_blocks(rows), block, 0, (cudaStream_t)stream>>>(in, out, rows, nz, ny, nx, factor);
     return finish("downsample_kernel");
 }
 
@@ -156,8 +195,9 @@ extern "C" int cbct_upsample(const float *in, float *out, int64_t n_outer, int32
                              int32_t factor, void *stream)
 {
     if (!in || !out || n_outer < 1 || factor < 1 || nz_in < 1 || ny_in < 1 || nx_in < 1) return CBCT_ERR_INVALID_ARG;
-    const size_t n = (size_t)n_outer * nz_in * ny_in * nx_in * factor * factor * factor;
-    upsample_kernel<<<blocks_for(n), 256, 0, (cudaStream_t)stream>>>(in, out, n, nz_in, ny_in, nx_in, factor);
+    const size_t rows = (size_t)n_outer * nz_in * ny_in;
+    const int vec4 = ((nx_in * factor) % 4 == 0) && ((uintptr_t)out % 16 == 0);
+    upsample_kernel<<<row_blocks(rows), dim3(64, 4), 0, (cudaStream_t)stream>>>(in, out, rows, nz_in, ny_in, nx_in, factor, vec4);
     return finish("upsample_kernel");
 }
 
@@ -167,7 +207,11 @@ extern "C" int cbct_proj_down(const float *in, float *out, int64_t n_outer, int3
     if (!in || !out || n_outer < 1 || factor < 1 || n_views_in < 1 || nv_in < 1 || nu_in < 1) return CBCT_ERR_INVALID_ARG;
     if (nv_in % factor || nu_in % factor) return CBCT_ERR_INVALID_ARG;
     const int n_views_out = (n_views_in + factor - 1) / factor, nv = nv_in / factor, nu = nu_in / factor;
-    const size_t n = (size_t)n_outer * n_views_out * nv * nu;
-    proj_down_kernel<<<blocks_for(n), 256, 0, (cudaStream_t)stream>>>(in, out, n, n_views_in, n_views_out, nv, nu, factor);
+    const size_t rows = (size_t)n_outer * n_views_out * nv;
+    const bool al = ((uintptr_t)in % 16 == 0);
+    const dim3 block(64, 4);
+    if (factor == 2 && al) proj_down_kernel<2><<<row_blocks(rows), block, 0, (cudaStream_t)stream>>>(in, out, rows, n_views_in, n_views_out, nv, nu, 2);
+    else if (factor == 4 && al) proj_down_kernel<4><<<row_blocks(rows), block, 0, (cudaStream_t)stream>>>(in, out, rows, n_views_in, n_views_out, nv, nu, 4);
+    else proj_down_kernel<0><<<row_blocks(rows), block, 0, (cudaStream_t)stream>>>(in, out, rows, n_views_in, n_views_out, nv, nu, factor);
     return finish("proj_down_kernel");
 }
