@@ -133,6 +133,15 @@ int cbct_redundancy_weight(const cbct_geom *g, const float *sino_in, float *sino
 /* The det_nu redundancy weights w(u) in fp64 (host; needs no CUDA device). */
 int cbct_geom_redundancy_weights(const cbct_geom *g, double *w_out);
 
+/* NEXT-3: fusions on the hot path of Alg. 1.
+ * cbct_fp_residual: sino = P vol - y, the argument of the Landweber term P*(P x - y); the subtraction happens in the
+ * projector's epilogue (y: DEVICE sinogram of the same layout, y != sino).
+ * cbct_bp_adjoint_weighted: vol = P^T (w(u) * sino), i.e. P*(w d) / P*(w y); the weighting is
+ * fused into the adjoint's sinogram re-layout pass.  Otherwise as cbct_fp / cbct_bp_adjoint. */
+int cbct_fp_residual(const cbct_geom *g, const float *vol, const float *y, float *sino, int32_t channels,
+                     void *cuda_stream);
+int cbct_bp_adjoint_weighted(const cbct_geom *g, const float *sino, float *vol, int32_t channels, void *cuda_stream);
+
 /* NEXT-2.  Field-of-view tensor: vol_out[z,y,x] = (number of views in which the
  * centre of voxel (z,y,x) projects onto the panel's active area, -1/2 <= fu < nu-1/2 and -1/2 <= fv < nv-1/2) /
  * n_views (reading R21).  vol_out: nz*ny*nx floats, DEVICE pointer, overwritten. */

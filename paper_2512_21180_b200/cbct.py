@@ -22,6 +22,7 @@ EXPORTS = (
     "cbct_geom_count_samples", "cbct_geom_num_slabs", "cbct_geom_launch_count",
     "cbct_geom_profile", "cbct_geom_profile_read",
     "cbct_fdk_filter", "cbct_redundancy_weight", "cbct_geom_redundancy_weights",
+    "cbct_fp_residual", "cbct_bp_adjoint_weighted",
     "cbct_fov", "cbct_downsample", "cbct_upsample", "cbct_proj_down",
     "cbct_status_string", "cbct_last_cuda_error",
 )
@@ -75,6 +76,8 @@ def load_library() -> ctypes.CDLL:
     L.cbct_fdk_filter.argtypes = [vp, vp, vp, i32, i32, vp]
     L.cbct_redundancy_weight.argtypes = [vp, vp, vp, i32, vp]
     L.cbct_geom_redundancy_weights.argtypes = [vp, ctypes.POINTER(ctypes.c_double)]
+    L.cbct_fp_residual.argtypes = [vp, vp, vp, vp, i32, vp]
+    L.cbct_bp_adjoint_weighted.argtypes = [vp, vp, vp, i32, vp]
     L.cbct_fov.argtypes = [vp, vp, vp]
     i64 = ctypes.c_int64
     L.cbct_downsample.argtypes = [vp, vp, i64, i32, i32, i32, i32, vp]
@@ -201,6 +204,20 @@ class Geometry:
         _check(load_library().cbct_geom_redundancy_weights(
             self._h, w.ctypes.data_as(ctypes.POINTER(ctypes.c_double))))
         return w
+
+    # --- NEXT-3: fused variants ------------------------------------------------
+    def fp_residual(self, vol, y, sino, channels: int = 1, stream=None):
+        """cbct_fp_residual: sino = P vol - y (y: device sinogram)."""
+        pv, py = _ptr_and_keep(vol, channels * self.n_vol), _ptr_and_keep(y, channels * self.n_sino)
+        ps = _ptr_and_keep(sino, channels * self.n_sino)
+        _check(load_library().cbct_fp_residual(self._h, pv, py, ps, channels, _stream_handle(stream)))
+        return sino
+
+    def bp_adjoint_weighted(self, sino, vol, channels: int = 1, stream=None):
+        """cbct_bp_adjoint_weighted: vol = P^T (w(u) * sino)."""
+        ps, pv = _ptr_and_keep(sino, channels * self.n_sino), _ptr_and_keep(vol, channels * self.n_vol)
+        _check(load_library().cbct_bp_adjoint_weighted(self._h, ps, pv, channels, _stream_handle(stream)))
+        return vol
 
     # --- NEXT-2: field-of-view tensor -----------------------------------------
     def fov(self, vol_out, stream=None):

@@ -50,7 +50,8 @@ struct AdjGeom {
 // (the NR views related by a grid rotation side by side, one vector load)
 template <int NR>
 __global__ void __launch_bounds__(256)
-interleave_views_kernel(const float *__restrict__ in, float *__restrict__ out, int nq, size_t img, int channels)
+interleave_views_kernel(const float *__restrict__ in, float *__restrict__ out, int nq, size_t img, int channels,
+                        const float *__restrict__ weights, int nu)
 {
     const size_t n = (size_t)channels * nq * img;
     for (size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x; e < n; e += (size_t)gridDim.x * blockDim.x) {
@@ -60,6 +61,11 @@ interleave_views_kernel(const float *__restrict__ in, float *__restrict__ out, i
         float vals[NR];
 #pragma unroll
         for (int r = 0; r < NR; ++r) vals[r] = __ldg(src + (size_t)r * nq * img);
+        if (weights) {  // w(u) of P*(w y), fused into the re-layout (NEXT-3)
+            const float w = __ldg(weights + pix % nu);
+#pragma unroll
+            for (int r = 0; r < NR; ++r) vals[r] *= w;
+        }
         if (NR == 4) reinterpret_cast<float4 *>(out)[e] = make_float4(vals[0], vals[1], vals[2], vals[NR - 1]);
         else if (NR == 2) reinterpret_cast<float2 *>(out)[e] = make_float2(vals[0], vals[NR - 1]);
         else out[e] = vals[0];
@@ -221,7 +227,8 @@ adjoint_gather_kernel(const float *__restrict__ sinoI, float *__restrict__ vol, 
 // ---------------------------------------------------------------------------
 // launchers
 // ---------------------------------------------------------------------------
-int cbct_launch_interleave_views(cbct_geom *g, const float *sino, float *out, int channels, cudaStream_t st)
+int cbct_launch_interleave_views(cbct_geom *g, const float *sino, float *out, int channels, const float *weights,
+                                 cudaStream_t st)
 {
     const int NR = g->sym_rot;
     const int nq = g->d.n_views / NR;
@@ -229,8 +236,8 @@ int cbct_launch_interleave_views(cbct_geom *g, const float *sino, float *out, in
     const size_t n = (size_t)channels * nq * img;
     size_t blocks = (n + 255) / 256;
     if (blocks > 148u * 16u) blocks = 148u * 16u;
-    if (NR == 4) interleave_views_kernel<4><<<(unsigned)blocks, 256, 0, st>>>(sino, out, nq, img, channels);
-    else if (NR == 2) interleave_views_kernel<2><<<(unsigned)blocks, 256, 0, st>>>(sino, out, nq, img, channels);
+    if (NR == 4) interleave_views_kernel<4><<<(unsigned)blocks, 256, 0, st>>>(sino, out, nq, img, channels, weights, g->d.det_nu);
+    else if (NR == 2) interleave_views_kernel<2><<<(unsigned)blocks, 256, 0, st>>>(sino, out, nq, img, channels, weights, g->d.det_nu);
     else return CBCT_ERR_INVALID_ARG;
     return cbct_check_launch(g, "interleave_views_kernel");
 }

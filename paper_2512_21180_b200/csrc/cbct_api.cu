@@ -88,11 +88,14 @@ static int begin_call(const cbct_geom *gc, const void *vol, const void *sino, in
 // ---------------------------------------------------------------------------
 // A2 + A5
 // ---------------------------------------------------------------------------
-extern "C" int cbct_fp(const cbct_geom *gc, const float *vol, float *sino, int32_t channels, void *stream)
+// y != nullptr: sino = P vol - y (the residual of the Landweber term, fused into the epilogue; y is a
+// DEVICE sinogram).  In the slab path the sinogram starts as -y instead of zero.
+static int fp_impl(const cbct_geom *gc, const float *vol, const float *y, float *sino, int32_t channels, void *stream)
 {
     CallCtx cx;
     int rc = begin_call(gc, vol, sino, channels, stream, cx);
     if (rc) return rc;
+    if (y && (classify(y) != MEM_DEVICE || y == sino)) return CBCT_ERR_INVALID_ARG;
     cbct_geom *g = cx.g;
     cudaStream_t st = cx.st;
     const int nz = g->d.vol_nz;
@@ -119,7 +122,13 @@ extern "C" int cbct_fp(const cbct_geom *gc, const float *vol, float *sino, int32
     }
     if (n_slabs > 1) {
         // every slab adds its part (only into the detector rows its shadow covers) to a zeroed sinogram
-        CBCT_CUDA_TRY(cudaMemsetAsync(d_sino, 0, cx.nsino * channels * sizeof(float), st));
+        if (y) {
+            CBCT_CUDA_TRY(cudaMemcpyAsync(d_sino, y, cx.nsino * channels * sizeof(float), cudaMemcpyDeviceToDevice, st));
+            rc = cbct_launch_negate(g, d_sino, cx.nsino * channels, st);
+            if (rc) return rc;
+        } else {
+            CBCT_CUDA_TRY(cudaMemsetAsync(d_sino, 0, cx.nsino * channels * sizeof(float), st));
+        }
         // the copy stream starts after everything already queued on `st`
         CBCT_CUDA_TRY(cudaEventRecord(g->ev[0], st));
         CBCT_CUDA_TRY(cudaStreamWaitEvent(g->copy_stream, g->ev[0], 0));
@@ -147,7 +156,7 @@ extern "C" int cbct_fp(const cbct_geom *gc, const float *vol, float *sino, int32
             CBCT_CUDA_TRY(cudaEventRecord(g->ev[b], cs));
             CBCT_CUDA_TRY(cudaStreamWaitEvent(st, g->ev[b], 0));
         }
-        rc = cbct_launch_fp(g, r, buf, d_sino, channels, n_slabs > 1, st);
+        rc = cbct_launch_fp(g, r, buf, d_sino, channels, n_slabs > 1, n_slabs > 1 ? nullptr : y, st);
         if (rc) return rc;
         if (n_slabs > 1) CBCT_CUDA_TRY(cudaEventRecord(g->ev[2 + b], st));
     }
@@ -155,6 +164,18 @@ extern "C" int cbct_fp(const cbct_geom *gc, const float *vol, float *sino, int32
         CBCT_CUDA_TRY(cudaMemcpyAsync(sino, d_sino, cx.nsino * channels * sizeof(float), cudaMemcpyDeviceToHost, st));
     if (cx.pageable) CBCT_CUDA_TRY(cudaStreamSynchronize(st));
     return CBCT_OK;
+}
+
+extern "C" int cbct_fp(const cbct_geom *gc, const float *vol, float *sino, int32_t channels, void *stream)
+{
+    return fp_impl(gc, vol, nullptr, sino, channels, stream);
+}
+
+extern "C" int cbct_fp_residual(const cbct_geom *gc, const float *vol, const float *y, float *sino, int32_t channels,
+                                void *stream)
+{
+    if (!y) return CBCT_ERR_INVALID_ARG;
+    return fp_impl(gc, vol, y, sino, channels, stream);
 }
 
 // ---------------------------------------------------------------------------
@@ -209,7 +230,7 @@ static int produce_volume(CallCtx &cx, float *vol, Launch launch)
 // ---------------------------------------------------------------------------
 // A3
 // ---------------------------------------------------------------------------
-extern "C" int cbct_bp_adjoint(const cbct_geom *gc, const float *sino, float *vol, int32_t channels, void *stream)
+static int adjoint_impl(const cbct_geom *gc, const float *sino, float *vol, int32_t channels, void *stream, bool weighted)
 {
     CallCtx cx;
     int rc = begin_call(gc, vol, sino, channels, stream, cx);
@@ -225,10 +246,20 @@ extern "C" int cbct_bp_adjoint(const cbct_geom *gc, const float *sino, float *vo
         CBCT_CUDA_TRY(cudaMemcpyAsync(g->ws_sino, sino, sino_bytes, cudaMemcpyHostToDevice, st));
         d_sino = g->ws_sino;
     }
-    if (g->sym_rot > 1) {  // views related by a grid rotation, interleaved for vector loads
+    if (weighted) {
+        rc = cbct_ensure_filter_tables(g);
+        if (rc) return rc;
+    }
+    if (g->sym_rot > 1) {  // views related by a grid rotation, interleaved for vector loads (+ w(u) if asked)
         rc = ensure(&g->ws_sino2, &g->ws_sino2_bytes, sino_bytes);
         if (rc) return rc;
-        rc = cbct_launch_interleave_views(g, d_sino, g->ws_sino2, channels, st);
+        rc = cbct_launch_interleave_views(g, d_sino, g->ws_sino2, channels, weighted ? g->d_filter_tab : nullptr, st);
+        if (rc) return rc;
+        d_sino = g->ws_sino2;
+    } else if (weighted) {  // no re-layout pass to fuse into: one weighting pass into workspace
+        rc = ensure(&g->ws_sino2, &g->ws_sino2_bytes, sino_bytes);
+        if (rc) return rc;
+        rc = cbct_launch_redundancy_weight(g, d_sino, g->ws_sino2, channels, st);
         if (rc) return rc;
         d_sino = g->ws_sino2;
     }
@@ -238,6 +269,17 @@ extern "C" int cbct_bp_adjoint(const cbct_geom *gc, const float *sino, float *vo
     if (rc) return rc;
     if (cx.pageable) CBCT_CUDA_TRY(cudaStreamSynchronize(st));
     return CBCT_OK;
+}
+
+extern "C" int cbct_bp_adjoint(const cbct_geom *gc, const float *sino, float *vol, int32_t channels, void *stream)
+{
+    return adjoint_impl(gc, sino, vol, channels, stream, false);
+}
+
+extern "C" int cbct_bp_adjoint_weighted(const cbct_geom *gc, const float *sino, float *vol, int32_t channels,
+                                        void *stream)
+{
+    return adjoint_impl(gc, sino, vol, channels, stream, true);
 }
 
 // ---------------------------------------------------------------------------

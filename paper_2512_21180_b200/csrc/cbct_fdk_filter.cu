@@ -116,7 +116,7 @@ extern "C" int cbct_geom_redundancy_weights(const cbct_geom *g, double *w_out)
 }
 
 // device tables: [0, nu) redundancy weights, [nu, 2nu) uniform 1/2, [2nu, 3nu) H[n] = dphi a h[n]
-static int ensure_filter_tables(cbct_geom *g, cudaStream_t st)
+int cbct_ensure_filter_tables(cbct_geom *g)
 {
     if (g->d_filter_tab) return CBCT_OK;
     const cbct_geom_desc &d = g->d;
@@ -136,7 +136,6 @@ static int ensure_filter_tables(cbct_geom *g, cudaStream_t st)
     CBCT_CUDA_TRY(cudaMalloc((void **)&g->d_filter_tab, tab.size() * sizeof(float)));
     // synchronous copy from a stack-lifetime vector; happens once per handle
     CBCT_CUDA_TRY(cudaMemcpy(g->d_filter_tab, tab.data(), tab.size() * sizeof(float), cudaMemcpyHostToDevice));
-    (void)st;
     return CBCT_OK;
 }
 
@@ -156,7 +155,7 @@ extern "C" int cbct_fdk_filter(const cbct_geom *gc, const float *sino_in, float 
     if (d.det_nu > 2048) return CBCT_ERR_UNSUPPORTED;  // 4 nu floats of shared memory per CTA
     if (!is_device_ptr(sino_in) || !is_device_ptr(sino_out)) return CBCT_ERR_INVALID_ARG;
     cudaStream_t st = (cudaStream_t)stream;
-    int rc = ensure_filter_tables(g, st);
+    int rc = cbct_ensure_filter_tables(g);
     if (rc) return rc;
     const int nu = d.det_nu;
     const size_t n_rows = (size_t)channels * d.n_views * d.det_nv;
@@ -172,14 +171,9 @@ extern "C" int cbct_fdk_filter(const cbct_geom *gc, const float *sino_in, float 
     return cbct_check_launch(g, "fdk_filter_kernel");
 }
 
-extern "C" int cbct_redundancy_weight(const cbct_geom *gc, const float *sino_in, float *sino_out, int32_t channels,
-                                      void *stream)
+int cbct_launch_redundancy_weight(cbct_geom *g, const float *sino_in, float *sino_out, int channels, cudaStream_t st)
 {
-    if (!gc || !sino_in || !sino_out || channels < 1) return CBCT_ERR_INVALID_ARG;
-    cbct_geom *g = const_cast<cbct_geom *>(gc);
-    if (!is_device_ptr(sino_in) || !is_device_ptr(sino_out)) return CBCT_ERR_INVALID_ARG;
-    cudaStream_t st = (cudaStream_t)stream;
-    int rc = ensure_filter_tables(g, st);
+    int rc = cbct_ensure_filter_tables(g);
     if (rc) return rc;
     const size_t n = (size_t)channels * g->d.n_views * g->d.det_nv * g->d.det_nu;
     size_t blocks = (n + 255) / 256;
@@ -194,4 +188,12 @@ extern "C" int cbct_redundancy_weight(const cbct_geom *gc, const float *sino_in,
         redundancy_weight_kernel<<<(unsigned)blocks, 256, 0, st>>>(sino_in, sino_out, g->d_filter_tab, g->d.det_nu, n);
     }
     return cbct_check_launch(g, "redundancy_weight_kernel");
+}
+
+extern "C" int cbct_redundancy_weight(const cbct_geom *gc, const float *sino_in, float *sino_out, int32_t channels,
+                                      void *stream)
+{
+    if (!gc || !sino_in || !sino_out || channels < 1) return CBCT_ERR_INVALID_ARG;
+    if (!is_device_ptr(sino_in) || !is_device_ptr(sino_out)) return CBCT_ERR_INVALID_ARG;
+    return cbct_launch_redundancy_weight(const_cast<cbct_geom *>(gc), sino_in, sino_out, channels, (cudaStream_t)stream);
 }

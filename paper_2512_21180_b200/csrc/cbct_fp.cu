@@ -111,7 +111,7 @@ template <int CB, int TU>
 __global__ void __launch_bounds__(FP_CTA_U *FP_CTA_V)
 fp_kernel(const float4 *__restrict__ packed, float *__restrict__ sino, const __grid_constant__ RayGeom G,
           const __grid_constant__ ViewChunk V, int view0, int accumulate, size_t packed_cstride,
-          size_t sino_cstride, int band0)
+          size_t sino_cstride, int band0, const float *__restrict__ sub)
 {
     constexpr int TV = 32 / TU, WU = FP_CTA_U / TU;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -148,11 +148,18 @@ fp_kernel(const float4 *__restrict__ packed, float *__restrict__ sino, const __g
 #pragma unroll
     for (int c = 0; c < CB; ++c) {
         float val = (acc[c] + acc2[c]) * delta;
+        if (sub) val -= __ldg(sub + c * sino_cstride + o);  // fused residual P x - y (NEXT-3)
         float *dst = sino + c * sino_cstride + o;
         *dst = accumulate ? *dst + val : val;
     }
 }
 
+
+__global__ void __launch_bounds__(256) negate_kernel(float *buf, size_t n)
+{
+    for (size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x; e < n; e += (size_t)gridDim.x * blockDim.x)
+        buf[e] = -buf[e];
+}
 
 // ---------------------------------------------------------------------------
 // launchers
@@ -172,18 +179,18 @@ int cbct_launch_pack_volume(cbct_geom *g, const RayGeom &r, const float *src, fl
 template <int CB>
 static int launch_fp_cb(cbct_geom *g, const RayGeom &r, const ViewChunk &vc, int nviews, int view0,
                         const float4 *packed, float *sino, int accumulate, size_t pstride, size_t sstride,
-                        int band0, int nbands, cudaStream_t st)
+                        int band0, int nbands, const float *sub, cudaStream_t st)
 {
     dim3 grid((r.nu + FP_CTA_U - 1) / FP_CTA_U, nviews, nbands);
     cbct_prof_begin(g, CBCT_KERNEL_FP, st);
     fp_kernel<CB, 4><<<grid, FP_CTA_U * FP_CTA_V, 0, st>>>(packed, sino, r, vc, view0, accumulate, pstride, sstride,
-                                                           band0);
+                                                           band0, sub);
     cbct_prof_end(g, CBCT_KERNEL_FP, st);
     return cbct_check_launch(g, "fp_kernel");
 }
 
 int cbct_launch_fp(cbct_geom *g, const RayGeom &r, const float4 *packed, float *sino, int channels, int accumulate,
-                   cudaStream_t st)
+                   const float *sub, cudaStream_t st)
 {
     const size_t pstride = cbct_packed_volume_cells(r);
     const size_t sstride = (size_t)g->d.n_views * r.nv * r.nu;
@@ -215,10 +222,18 @@ int cbct_launch_fp(cbct_geom *g, const RayGeom &r, const float4 *packed, float *
             const float4 *p = packed + c * pstride;
             float *s = sino + c * sstride;
             // 2 channels per thread measured best at 256^3 (4 lowers occupancy and L1 hit rate)
-            if (left >= 2) { rc = launch_fp_cb<2>(g, r, vc, n, view0, p, s, accumulate, pstride, sstride, band0, nbands, st); c += 2; }
-            else { rc = launch_fp_cb<1>(g, r, vc, n, view0, p, s, accumulate, pstride, sstride, band0, nbands, st); c += 1; }
+            if (left >= 2) { rc = launch_fp_cb<2>(g, r, vc, n, view0, p, s, accumulate, pstride, sstride, band0, nbands, sub ? sub + c * sstride : nullptr, st); c += 2; }
+            else { rc = launch_fp_cb<1>(g, r, vc, n, view0, p, s, accumulate, pstride, sstride, band0, nbands, sub ? sub + c * sstride : nullptr, st); c += 1; }
             if (rc) return rc;
         }
     }
     return CBCT_OK;
+}
+
+int cbct_launch_negate(cbct_geom *g, float *buf, size_t n, cudaStream_t st)
+{
+    size_t blocks = (n + 255) / 256;
+    if (blocks > 148u * 16u) blocks = 148u * 16u;
+    negate_kernel<<<(unsigned)blocks, 256, 0, st>>>(buf, n);
+    return cbct_check_launch(g, "negate_kernel");
 }

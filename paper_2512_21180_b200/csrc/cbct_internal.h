@@ -100,11 +100,17 @@ void cbct_prof_end(cbct_geom *g, int kernel, cudaStream_t st);
 // quad-pack: src[C][nz_src][ny][nx] planes [r.z0, r.z1) -> dst[C][pz][py][px] float4 cells (cbct_fp.cu)
 int cbct_launch_pack_volume(cbct_geom *g, const RayGeom &r, const float *src, float4 *dst, int channels,
                             size_t src_channel_stride, int src_z_origin, cudaStream_t st);
-// forward projection of the packed slab(s); accumulate != 0 adds into sino
+// forward projection of the packed slab(s); accumulate != 0 adds into sino; sub != nullptr: minus sub (same layout)
 int cbct_launch_fp(cbct_geom *g, const RayGeom &r, const float4 *packed, float *sino, int channels,
-                   int accumulate, cudaStream_t st);
-// view-interleaved copy of the sinogram for the gather adjoint (only if g->sym_rot > 1)
-int cbct_launch_interleave_views(cbct_geom *g, const float *sino, float *out, int channels, cudaStream_t st);
+                   int accumulate, const float *sub, cudaStream_t st);
+// view-interleaved copy of the sinogram for the gather adjoint (only if g->sym_rot > 1);
+// weights != nullptr: every pixel is multiplied by weights[iu] on the way (NEXT-3)
+int cbct_launch_interleave_views(cbct_geom *g, const float *sino, float *out, int channels, const float *weights,
+                                 cudaStream_t st);
+// device tables of the FDK front end (cbct_fdk_filter.cu): g->d_filter_tab[0, nu) = redundancy weights
+int cbct_ensure_filter_tables(cbct_geom *g);
+int cbct_launch_negate(cbct_geom *g, float *buf, size_t n, cudaStream_t st);  // buf = -buf (cbct_fp.cu)
+int cbct_launch_redundancy_weight(cbct_geom *g, const float *in, float *out, int channels, cudaStream_t st);
 // gather adjoint into vol planes [zs0, zs1)
 int cbct_launch_adjoint(cbct_geom *g, const float *sino_src, float *vol, int channels, int zs0, int zs1,
                         size_t vol_channel_stride, int vol_z_origin, cudaStream_t st);

@@ -479,3 +479,27 @@ def test_next2_resampling(cbct, oracle_mod):
         assert np.max(np.abs(out.cpu().numpy() - oracle_mod.proj_down(p.astype(np.float64), f))) <= 1e-6
     with pytest.raises(cbct.CbctError):
         cbct.downsample(dev(z), torch.empty((3, 2, 4, 6), device="cuda"), 3)
+
+
+@pytest.mark.parametrize("over,cap", [(dict(), 0), (dict(n_views=10, vol_nx=30, det_off_u_mm=20.0), 0),
+                                      (dict(n_views=7, det_off_u_mm=-15.0), 0), (dict(vol_nz=40, n_views=12, det_off_u_mm=15.0), 2500000)])
+def test_next3_fused_residual_and_weighted_adjoint(cbct, oracle_mod, over, cap):
+    """NEXT-3: cbct_fp_residual = P x - y and cbct_bp_adjoint_weighted = P^T (w y), against the oracle's
+    compositions (resident and z-slab paths; rotation-interleaved and plain sinogram layouts)."""
+    kw = dict(synth.geom_kwargs(synth.CONFIGS["tiny"]))
+    kw.update(over)
+    g = cbct.Geometry(**kw, max_workset_bytes=cap)
+    og = oracle_mod.Geom(**kw)
+    rng = np.random.default_rng(31)
+    x = rng.random((3,) + g.vol_shape, dtype=np.float32)
+    y = rng.random((3,) + g.sino_shape, dtype=np.float32)
+    out = torch.full((3,) + g.sino_shape, float("nan"), device="cuda")
+    g.fp_residual(dev(x), dev(y), out, 3)
+    Ax = oracle_mod.fp(og, x.astype(np.float64))
+    res = out.cpu().numpy().astype(np.float64)
+    assert np.linalg.norm(res - (Ax - y)) <= 1e-5 * np.linalg.norm(Ax)   # error relative to the size of P x
+    vol = torch.full((3,) + g.vol_shape, float("nan"), device="cuda")
+    g.bp_adjoint_weighted(dev(y), vol, 3)
+    torch.cuda.synchronize()
+    want = oracle_mod.bp_adjoint(og, y.astype(np.float64) * oracle_mod.redundancy_weight(og))
+    assert rel_l2(vol.cpu().numpy().astype(np.float64), want) <= 1e-4
