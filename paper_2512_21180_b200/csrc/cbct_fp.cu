@@ -183,8 +183,14 @@ static int launch_fp_cb(cbct_geom *g, const RayGeom &r, const ViewChunk &vc, int
 {
     dim3 grid((r.nu + FP_CTA_U - 1) / FP_CTA_U, nviews, nbands);
     cbct_prof_begin(g, CBCT_KERNEL_FP, st);
-    fp_kernel<CB, 4><<<grid, FP_CTA_U * FP_CTA_V, 0, st>>>(packed, sino, r, vc, view0, accumulate, pstride, sstride,
-                                                           band0, sub);
+    // 4 x 8-pixel warps suit the bank swizzle best when rays cross the whole volume; in a thin z-slab
+    // (streaming) 8 x 4-pixel warps keep the lanes' in-slab segments alike (measured on config 5: +17 %)
+    if (r.z1 - r.z0 >= 64 || r.z1 - r.z0 == r.nz)
+        fp_kernel<CB, 4><<<grid, FP_CTA_U * FP_CTA_V, 0, st>>>(packed, sino, r, vc, view0, accumulate, pstride, sstride,
+                                                               band0, sub);
+    else
+        fp_kernel<CB, 8><<<grid, FP_CTA_U * FP_CTA_V, 0, st>>>(packed, sino, r, vc, view0, accumulate, pstride, sstride,
+                                                               band0, sub);
     cbct_prof_end(g, CBCT_KERNEL_FP, st);
     return cbct_check_launch(g, "fp_kernel");
 }
