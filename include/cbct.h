@@ -12,10 +12,13 @@
  *   multi-channel use       PAPER.md:167, :221, :227, :230 (Alg. 1 l.16-19)
  *   multi-scale use         PAPER.md:270 (one handle per scale / view subset)
  *   streaming               PAPER.md:165, :292 (data kept on the host, parts sent to the GPU)
+ *   beyond the four core calls (SURVEY.md s.8(f) NEXT-1..3): the FDK_w front end and redundancy
+ *   weight w, the field-of-view tensor V, Downsample /
+ *   Upsample / ProjDown and the fused P x - y / P^T(w y) of Alg. 1 l.18-19
  *
  * The paper defines P only as a continuous integral; the discretisation is
  * the one BASELINE.json names (ray-driven, trilinear samples at a fixed step)
- * with the readings R1-R11 listed in DESIGN.md section 3.
+ * with the readings R1-R22 listed in DESIGN.md section 3.
  *
  * Conventions
  *   - World frame (mm): isocentre at the origin, rotation axis +z.  View i has
