@@ -256,7 +256,8 @@ int cbct_launch_fdk(cbct_geom *g, const float *padded_sino, float *vol, int chan
     G.bz0 = zs0; G.bz1 = mirror ? (d.vol_nz + 1) / 2 : zs1;
     G.n_views = 0; G.nbase = 0;
     const size_t vs = vol_channel_stride;
-    if (NR == 4) return mirror ? launch_fdk<4, 2, 4>(g, G, padded_sino, vol, channels, vs, vol_z_origin, st)
+    // z per thread: 3 measured best for the 8-voxel variant (1: 6.3 ms, 2: 4.8, 3: 4.6, 4: 5.2, 8: 5.3 per channel)
+    if (NR == 4) return mirror ? launch_fdk<4, 2, 3>(g, G, padded_sino, vol, channels, vs, vol_z_origin, st)
                                : launch_fdk<4, 1, 8>(g, G, padded_sino, vol, channels, vs, vol_z_origin, st);
     if (NR == 2) return mirror ? launch_fdk<2, 2, 8>(g, G, padded_sino, vol, channels, vs, vol_z_origin, st)
                                : launch_fdk<2, 1, 8>(g, G, padded_sino, vol, channels, vs, vol_z_origin, st);
