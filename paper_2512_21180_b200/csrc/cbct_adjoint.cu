@@ -44,6 +44,10 @@ struct AdjGeom {
     int bz0, bz1;                           // base planes [bz0, bz1)
     int nq;                                 // views in this launch
     int nbase;                              // n_views / NR: views i and i + nbase differ by 360/NR degrees
+    // small grids do not fill the GPU with one thread per base voxel: the views of a launch are then split
+    // over `nsplit` groups of CTAs, each writing its partial sums to its own copy of the output
+    int nsplit, views_per_split;
+    size_t split_stride;                    // floats between the partial outputs of consecutive splits
 };
 
 // out[c][iq][iv][iu][p] = in[c][iq + p nq][iv][iu], iq < nq = n_views / NR
@@ -86,8 +90,12 @@ adjoint_gather_kernel(const float *__restrict__ sinoI, float *__restrict__ vol, 
 {
     const int ix = blockIdx.x * ADJ_BX + threadIdx.x;
     const int iy = blockIdx.y * ADJ_BY + threadIdx.y;
-    const int iz = G.bz0 + blockIdx.z * ADJ_BZ + threadIdx.z;
+    const int nzb = (G.bz1 - G.bz0 + ADJ_BZ - 1) / ADJ_BZ;
+    const int split = blockIdx.z / nzb;
+    const int iz = G.bz0 + (blockIdx.z - split * nzb) * ADJ_BZ + threadIdx.z;
     if (ix >= G.bx || iy >= G.by || iz >= G.bz1) return;
+    vol += split * G.split_stride;
+    const int q_begin = split * G.views_per_split, q_end = min(G.nq, q_begin + G.views_per_split);
     const double X = G.x0 + ix, Y = G.y0 + iy, Z = G.z0 + iz;
     float acc[NM][CB][NR];
 #pragma unroll
@@ -101,7 +109,7 @@ adjoint_gather_kernel(const float *__restrict__ sinoI, float *__restrict__ vol, 
     const float zcull = 1.4143f * (float)G.inv_sdd;
     const size_t img = (size_t)G.nv * G.nu;
 
-    for (int q = 0; q < G.nq; ++q) {
+    for (int q = q_begin; q < q_end; ++q) {
         // ---- fp64 set-up of the voxel's projection (once per voxel and view) ----
         const double c = V.cs[q].x, s = V.cs[q].y;
         const double U = G.sid - (X * c + Y * s), w = Y * c - X * s;
@@ -242,15 +250,49 @@ int cbct_launch_interleave_views(cbct_geom *g, const float *sino, float *out, in
     return cbct_check_launch(g, "interleave_views_kernel");
 }
 
+// out[c][e] (+)= sum_s partial[s][c][e], fixed order (deterministic)
+__global__ void __launch_bounds__(256)
+reduce_splits_kernel(const float *__restrict__ partial, float *__restrict__ out, size_t n, int cb, int nsplit,
+                     size_t out_cstride)
+{
+    for (size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x; e < n * cb; e += (size_t)gridDim.x * blockDim.x) {
+        const size_t c = e / n, v = e - c * n;
+        float acc = 0.f;
+        for (int s = 0; s < nsplit; ++s) acc += __ldg(partial + ((size_t)s * cb + c) * n + v);
+        out[c * out_cstride + v] = acc;
+    }
+}
+
 template <int NR, int NM, int CB>
 static int launch_gather(cbct_geom *g, AdjGeom &G, const float *sinoI, float *vol, int accumulate_first,
-                         size_t sstride, size_t vstride, int vol_z_origin, cudaStream_t st)
+                         size_t sstride, size_t vstride, int vol_z_origin, float *partial, int nsplit, cudaStream_t st)
 {
     const int nq_total = g->d.n_views;
     G.nbase = g->d.n_views / NR;
     ViewChunk vc;
     dim3 block(ADJ_BX, ADJ_BY, ADJ_BZ);
-    dim3 grid((G.bx + ADJ_BX - 1) / ADJ_BX, (G.by + ADJ_BY - 1) / ADJ_BY, (G.bz1 - G.bz0 + ADJ_BZ - 1) / ADJ_BZ);
+    const int nzb = (G.bz1 - G.bz0 + ADJ_BZ - 1) / ADJ_BZ;
+    dim3 grid((G.bx + ADJ_BX - 1) / ADJ_BX, (G.by + ADJ_BY - 1) / ADJ_BY, nzb);
+    G.nsplit = 1; G.views_per_split = CBCT_VIEWS_PER_LAUNCH; G.split_stride = 0;
+    if (partial && nsplit > 1 && nq_total <= CBCT_VIEWS_PER_LAUNCH) {
+        // one launch, views split over groups of CTAs into partial outputs of the whole grid, then reduced
+        const size_t nvox = (size_t)G.nx * G.ny * G.nz;
+        for (int i = 0; i < nq_total; ++i) vc.cs[i] = make_double2(g->cosphi[i], g->sinphi[i]);
+        G.nq = nq_total;
+        G.nsplit = nsplit;
+        G.views_per_split = (nq_total + nsplit - 1) / nsplit;
+        G.split_stride = (size_t)CB * nvox;
+        grid.z = nzb * nsplit;
+        cbct_prof_begin(g, CBCT_KERNEL_ADJOINT, st);
+        adjoint_gather_kernel<NR, NM, CB><<<grid, block, 0, st>>>(sinoI, partial, G, vc, 0, 0, sstride, nvox, 0);
+        cbct_prof_end(g, CBCT_KERNEL_ADJOINT, st);
+        int rc = cbct_check_launch(g, "adjoint_gather_kernel");
+        if (rc) return rc;
+        size_t blocks = (nvox * CB + 255) / 256;
+        if (blocks > 148u * 16u) blocks = 148u * 16u;
+        reduce_splits_kernel<<<(unsigned)blocks, 256, 0, st>>>(partial, vol, nvox, CB, nsplit, vstride);
+        return cbct_check_launch(g, "reduce_splits_kernel");
+    }
     for (int q0 = 0; q0 < nq_total; q0 += CBCT_VIEWS_PER_LAUNCH) {
         int n = nq_total - q0;
         if (n > CBCT_VIEWS_PER_LAUNCH) n = CBCT_VIEWS_PER_LAUNCH;
@@ -268,7 +310,8 @@ static int launch_gather(cbct_geom *g, AdjGeom &G, const float *sinoI, float *vo
 
 template <int NR, int NM>
 static int launch_gather_channels(cbct_geom *g, AdjGeom &G, const float *sinoI, float *vol, int channels,
-                                  size_t sstride, size_t vstride, int vol_z_origin, cudaStream_t st)
+                                  size_t sstride, size_t vstride, int vol_z_origin, float *partial, int nsplit,
+                                  cudaStream_t st)
 {
     int c = 0;
     while (c < channels) {
@@ -276,8 +319,8 @@ static int launch_gather_channels(cbct_geom *g, AdjGeom &G, const float *sinoI, 
         const float *s = sinoI + c * sstride;
         float *v = vol + c * vstride;
         // 2 channels per thread: 4 needs 128 registers and measured slower (158 vs 143 ms at C = 8)
-        if (left >= 2 && NR * NM <= 8) { rc = launch_gather<NR, NM, 2>(g, G, s, v, 0, sstride, vstride, vol_z_origin, st); c += 2; }
-        else { rc = launch_gather<NR, NM, 1>(g, G, s, v, 0, sstride, vstride, vol_z_origin, st); c += 1; }
+        if (left >= 2 && NR * NM <= 8) { rc = launch_gather<NR, NM, 2>(g, G, s, v, 0, sstride, vstride, vol_z_origin, partial, nsplit, st); c += 2; }
+        else { rc = launch_gather<NR, NM, 1>(g, G, s, v, 0, sstride, vstride, vol_z_origin, partial, nsplit, st); c += 1; }
         if (rc) return rc;
     }
     return CBCT_OK;
@@ -287,9 +330,26 @@ static int launch_gather_channels(cbct_geom *g, AdjGeom &G, const float *sinoI, 
 // view-interleaved copy made by cbct_launch_interleave_views.  Writes planes
 // [zs0, zs1) of vol (whose first stored plane is vol_z_origin).  The z-mirror
 // is used only when the launch covers the whole grid.
-int cbct_launch_adjoint(cbct_geom *g, const float *sino_src, float *vol, int channels, int zs0, int zs1,
-                        size_t vol_channel_stride, int vol_z_origin, cudaStream_t st)
+// Number of view groups the adjoint uses for this geometry (1 = no splitting): enough to give the GPU
+// about a million threads when one thread per base voxel would not.
+int cbct_adjoint_view_splits(const cbct_geom *g)
 {
+    const cbct_geom_desc &d = g->d;
+    if (d.n_views > CBCT_VIEWS_PER_LAUNCH) return 1;
+    size_t threads = (size_t)d.vol_nx * d.vol_ny * d.vol_nz / ((size_t)g->sym_rot * (g->sym_mirror_z ? 2 : 1));
+    if (threads == 0) threads = 1;
+    size_t s = (2000000 + threads - 1) / threads;
+    if (s > 32) s = 32;
+    if (s > (size_t)d.n_views / 8) s = (size_t)d.n_views / 8;
+    return s < 1 ? 1 : (int)s;
+}
+
+// `partial` (nsplit > 1 only): workspace of nsplit * 2 * nx * ny * nz floats; used when the launch covers the
+// whole grid (zs0 = 0, zs1 = nz, vol_z_origin = 0).
+int cbct_launch_adjoint(cbct_geom *g, const float *sino_src, float *vol, int channels, int zs0, int zs1,
+                        size_t vol_channel_stride, int vol_z_origin, float *partial, int nsplit, cudaStream_t st)
+{
+    if (zs0 != 0 || zs1 != g->d.vol_nz || vol_z_origin != 0) { partial = nullptr; nsplit = 1; }
     const cbct_geom_desc &d = g->d;
     const double h = d.vox_mm;
     AdjGeom G;
@@ -313,12 +373,12 @@ int cbct_launch_adjoint(cbct_geom *g, const float *sino_src, float *vol, int cha
     G.nq = 0;
     const size_t sstride = (size_t)d.n_views * d.det_nv * d.det_nu;
     if (NR == 4) {
-        return mirror ? launch_gather_channels<4, 2>(g, G, sino_src, vol, channels, sstride, vol_channel_stride, vol_z_origin, st)
-                      : launch_gather_channels<4, 1>(g, G, sino_src, vol, channels, sstride, vol_channel_stride, vol_z_origin, st);
+        return mirror ? launch_gather_channels<4, 2>(g, G, sino_src, vol, channels, sstride, vol_channel_stride, vol_z_origin, partial, nsplit, st)
+                      : launch_gather_channels<4, 1>(g, G, sino_src, vol, channels, sstride, vol_channel_stride, vol_z_origin, partial, nsplit, st);
     } else if (NR == 2) {
-        return mirror ? launch_gather_channels<2, 2>(g, G, sino_src, vol, channels, sstride, vol_channel_stride, vol_z_origin, st)
-                      : launch_gather_channels<2, 1>(g, G, sino_src, vol, channels, sstride, vol_channel_stride, vol_z_origin, st);
+        return mirror ? launch_gather_channels<2, 2>(g, G, sino_src, vol, channels, sstride, vol_channel_stride, vol_z_origin, partial, nsplit, st)
+                      : launch_gather_channels<2, 1>(g, G, sino_src, vol, channels, sstride, vol_channel_stride, vol_z_origin, partial, nsplit, st);
     }
-    return mirror ? launch_gather_channels<1, 2>(g, G, sino_src, vol, channels, sstride, vol_channel_stride, vol_z_origin, st)
-                  : launch_gather_channels<1, 1>(g, G, sino_src, vol, channels, sstride, vol_channel_stride, vol_z_origin, st);
+    return mirror ? launch_gather_channels<1, 2>(g, G, sino_src, vol, channels, sstride, vol_channel_stride, vol_z_origin, partial, nsplit, st)
+                  : launch_gather_channels<1, 1>(g, G, sino_src, vol, channels, sstride, vol_channel_stride, vol_z_origin, partial, nsplit, st);
 }

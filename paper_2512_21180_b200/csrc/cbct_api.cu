@@ -263,8 +263,16 @@ static int adjoint_impl(const cbct_geom *gc, const float *sino, float *vol, int3
         if (rc) return rc;
         d_sino = g->ws_sino2;
     }
+    // small grids: split the views over groups of CTAs (partial outputs in workspace, then reduced)
+    int nsplit = cx.kv == MEM_DEVICE ? cbct_adjoint_view_splits(g) : 1;
+    float *partial = nullptr;
+    if (nsplit > 1) {
+        rc = ensure(&g->ws_vol, &g->ws_vol_bytes, (size_t)nsplit * 2 * cx.nvol * sizeof(float));
+        if (rc) return rc;
+        partial = g->ws_vol;
+    }
     rc = produce_volume(cx, vol, [&](float *dst, int zs0, int zs1, size_t cstride, int z_origin) {
-        return cbct_launch_adjoint(g, d_sino, dst, channels, zs0, zs1, cstride, z_origin, st);
+        return cbct_launch_adjoint(g, d_sino, dst, channels, zs0, zs1, cstride, z_origin, partial, nsplit, st);
     });
     if (rc) return rc;
     if (cx.pageable) CBCT_CUDA_TRY(cudaStreamSynchronize(st));

@@ -113,7 +113,8 @@ int cbct_launch_negate(cbct_geom *g, float *buf, size_t n, cudaStream_t st);  //
 int cbct_launch_redundancy_weight(cbct_geom *g, const float *in, float *out, int channels, cudaStream_t st);
 // gather adjoint into vol planes [zs0, zs1)
 int cbct_launch_adjoint(cbct_geom *g, const float *sino_src, float *vol, int channels, int zs0, int zs1,
-                        size_t vol_channel_stride, int vol_z_origin, cudaStream_t st);
+                        size_t vol_channel_stride, int vol_z_origin, float *partial, int nsplit, cudaStream_t st);
+int cbct_adjoint_view_splits(const cbct_geom *g);  // view groups for small grids (1 = none)
 int cbct_launch_pad_sino(cbct_geom *g, const float *src, float *dst, int channels, cudaStream_t st);
 // FDK backprojection from the padded sinogram into vol planes [zs0, zs1)
 int cbct_launch_fdk(cbct_geom *g, const float *padded_sino, float *vol, int channels, int zs0, int zs1,
