@@ -52,6 +52,72 @@ fdk_filter_kernel(const float *__restrict__ in, float *__restrict__ out, const f
     }
 }
 
+// Register-tiled variant for nu % 8 == 0: a thread owns 8 consecutive outputs, as two interleaved sets of 4
+// (even / odd columns).  For a set with outputs j0 + 2i the inputs of tap n+2 are those of tap n shifted by one
+// output (c[j0+2i-(n+2)] = c[j0+2(i-1)-n]), so each step loads only one new value on each side and reuses the
+// other three from registers: 2 LDS + 1 broadcast tap per 8 multiply-adds instead of 3 per 2.
+template <int DUMMY>
+__global__ void __launch_bounds__(256)
+fdk_filter8_kernel(const float *__restrict__ in, float *__restrict__ out, const float *__restrict__ tab_w,
+                   const float *__restrict__ tab_h, int nu, int nv, size_t n_rows, float u0, float du, float v0,
+                   float dv, float sdd)
+{
+    extern __shared__ float smem[];
+    const int tpr = blockDim.x, rpc = blockDim.y;      // threads per row, rows per CTA
+    // zeros | row | zeros; one pad word per 32 (element J sits at J + J/32): a thread's columns are 8 apart,
+    // and without the padding lanes t and t + 4 would hit the same bank
+    const int span = 3 * nu + 16, base = nu + 8, pitch = span + span / 32 + 1;
+    float *taps = smem;                                 // [nu]
+    float *rowbuf = smem + nu + (size_t)threadIdx.y * pitch;
+#define PADIDX(J) ((J) + ((J) >> 5))
+    for (int j = threadIdx.y * tpr + threadIdx.x; j < nu; j += tpr * rpc) taps[j] = tab_h[j];
+    for (int j = threadIdx.x; j < pitch; j += tpr) rowbuf[j] = 0.f;
+    const float h0 = tab_h[0];
+    for (size_t r0 = (size_t)blockIdx.x * rpc; r0 < n_rows; r0 += (size_t)gridDim.x * rpc) {
+        const size_t r = r0 + threadIdx.y;
+        __syncthreads();  // previous rows consumed; aprons / taps written
+        if (r < n_rows) {
+            const float v = fmaf((float)(r % nv), dv, v0);
+            const float s2 = fmaf(v, v, sdd * sdd);
+            for (int j = threadIdx.x; j < nu; j += tpr) {
+                const float u = fmaf((float)j, du, u0);
+                rowbuf[PADIDX(base + j)] = in[r * nu + j] * (tab_w[j] * sdd * rsqrtf(fmaf(u, u, s2)));
+            }
+        }
+        __syncthreads();
+        if (r >= n_rows) continue;
+        float res[8];
+#pragma unroll
+        for (int set = 0; set < 2; ++set) {
+            const int c0 = base + 8 * threadIdx.x + set;  // outputs at columns c0, c0 + 2, c0 + 4, c0 + 6
+            float acc[4], L[4], R[4];
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                acc[i] = h0 * rowbuf[PADIDX(c0 + 2 * i)];
+                L[i] = rowbuf[PADIDX(c0 + 2 * i - 1)];
+                R[i] = rowbuf[PADIDX(c0 + 2 * i + 1)];
+            }
+            for (int n = 1; n < nu; n += 8) {
+#pragma unroll
+                for (int u4 = 0; u4 < 4; ++u4) {  // tap n + 2 u4; logical L[i] lives in L[(i - u4) & 3], R[i] in R[(i + u4) & 3]
+                    const float h = taps[n + 2 * u4];
+#pragma unroll
+                    for (int i = 0; i < 4; ++i) acc[i] = fmaf(h, L[(i - u4) & 3] + R[(i + u4) & 3], acc[i]);
+                    const int jl = c0 - (n + 2 * u4) - 2, jr = c0 + 6 + (n + 2 * u4) + 2;
+                    L[(3 - u4) & 3] = rowbuf[PADIDX(jl)];          // new logical L[0] of the next tap
+                    R[u4 & 3] = rowbuf[PADIDX(jr)];                // new logical R[3] of the next tap
+                }
+            }
+#pragma unroll
+            for (int i = 0; i < 4; ++i) res[2 * i + set] = acc[i];
+        }
+        float4 *dst = reinterpret_cast<float4 *>(out + r * nu + 8 * threadIdx.x);
+        dst[0] = make_float4(res[0], res[1], res[2], res[3]);
+        dst[1] = make_float4(res[4], res[5], res[6], res[7]);
+    }
+#undef PADIDX
+}
+
 // out = w(u) * in   (P*(w y); in place allowed)
 __global__ void __launch_bounds__(256)
 redundancy_weight_kernel(const float *in, float *out, const float *__restrict__ tab_w, int nu,
@@ -163,6 +229,19 @@ extern "C" int cbct_fdk_filter(const cbct_geom *gc, const float *sino_in, float 
     const size_t smem = 4 * (size_t)nu * sizeof(float);
     const unsigned grid = (unsigned)(n_rows < 148u * 8u ? n_rows : 148u * 8u);
     // coordinates in mm here (the weights only need ratios)
+    const float fu0 = (float)(-0.5 * (nu - 1) * d.det_du_mm + d.det_off_u_mm);
+    const float fv0 = (float)(-0.5 * (d.det_nv - 1) * d.det_dv_mm + d.det_off_v_mm);
+    if (nu % 8 == 0 && (uintptr_t)sino_out % 16 == 0) {
+        const int tpr = nu / 8, rpc = 256 / tpr < 1 ? 1 : 256 / tpr;
+        const int span = 3 * nu + 16;
+        const size_t smem8 = ((size_t)nu + (size_t)rpc * (span + span / 32 + 1)) * sizeof(float);
+        const size_t want = (n_rows + rpc - 1) / rpc;
+        const unsigned grid8 = (unsigned)(want < 148u * 8u ? want : 148u * 8u);
+        fdk_filter8_kernel<0><<<grid8, dim3(tpr, rpc), smem8, st>>>(sino_in, sino_out, tw, g->d_filter_tab + 2 * (size_t)nu,
+                                                                  nu, d.det_nv, n_rows, fu0, (float)d.det_du_mm, fv0,
+                                                                  (float)d.det_dv_mm, (float)d.sdd_mm);
+        return cbct_check_launch(g, "fdk_filter8_kernel");
+    }
     fdk_filter_kernel<<<grid, 256, smem, st>>>(sino_in, sino_out, tw, g->d_filter_tab + 2 * (size_t)nu, nu, d.det_nv, n_rows,
                                                (float)(-0.5 * (nu - 1) * d.det_du_mm + d.det_off_u_mm),
                                                (float)d.det_du_mm,
