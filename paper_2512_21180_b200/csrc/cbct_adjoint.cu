@@ -171,8 +171,8 @@ adjoint_gather_kernel(const float *__restrict__ sinoI, float *__restrict__ vol, 
                 const float d0 = klo - fmaf(lamUf, invg, -0.5f);  // k - kU
                 float ex = fmaf(d0, gNx, Ax), ey = fmaf(d0, gNy, Ay), ez = fmaf(d0, gv, av);
                 float W = 0.f;
-                // the window holds at most 4 sqrt 2 < 6 samples (5 always evaluated, the 6th only when the window
-                // reaches it); samples past the window have weight 0 (clamps)
+                // the window is 2 sqrt 2 / step samples wide at most: < 6 for step >= 1/2 (5 always evaluated,
+                // the 6th only when the window reaches it); samples past the window have weight 0 (clamps)
 #pragma unroll
                 for (int j = 0; j < 6; ++j) {
                     const float wx = fmaxf(1.0f - fabsf(ex), 0.f);
@@ -181,6 +181,16 @@ adjoint_gather_kernel(const float *__restrict__ sinoI, float *__restrict__ vol, 
                     W = fmaf(wx * wy, wz, W);
                     if (j == 4 && fmaf(lam_hi, invg, -5.5f) <= klo) break;  // k = klo + 5 is past the window
                     ex += gNx; ey += gNy; ez += gv;
+                }
+                if (G.step < 0.5f) {  // finer steps: walk the rest of the window (uniform branch)
+                    const float kend = fmaf(lam_hi, invg, -0.5f);  // samples with k < kend are inside
+                    for (float kf = klo + 6.0f; kf < kend; kf += 1.0f) {
+                        const float wx = fmaxf(1.0f - fabsf(ex), 0.f);
+                        const float wy = fmaxf(1.0f - fabsf(ey), 0.f);
+                        const float wz = fmaxf(1.0f - fabsf(ez), 0.f);
+                        W = fmaf(wx * wy, wz, W);
+                        ex += gNx; ey += gNy; ez += gv;
+                    }
                 }
                 if (W == 0.f) continue;
 #pragma unroll

@@ -503,3 +503,14 @@ def test_next3_fused_residual_and_weighted_adjoint(cbct, oracle_mod, over, cap):
     torch.cuda.synchronize()
     want = oracle_mod.bp_adjoint(og, y.astype(np.float64) * oracle_mod.redundancy_weight(og))
     assert rel_l2(vol.cpu().numpy().astype(np.float64), want) <= 1e-4
+
+
+@pytest.mark.parametrize("step", [0.2, 0.37, 0.75, 1.0])
+def test_other_ray_steps(cbct, oracle_mod, step):
+    """step_vox other than 1/2 (the gather adjoint's sample window holds 2 sqrt 2 / step lattice points)."""
+    kw = dict(synth.geom_kwargs(synth.CONFIGS["tiny"]))
+    kw.update(step_vox=step, n_views=12, det_off_u_mm=18.0)
+    rng = np.random.default_rng(41)
+    vol = rng.random((2, 32, 32, 32), dtype=np.float32)
+    sino = rng.random((2, 12, 48, 48), dtype=np.float32)
+    check_all_three(cbct, oracle_mod, kw, vol, sino, "step %g" % step)
