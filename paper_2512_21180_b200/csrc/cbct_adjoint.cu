@@ -82,7 +82,7 @@ interleave_views_kernel(const float *__restrict__ in, float *__restrict__ out, i
 #define ADJ_BY 16
 #define ADJ_BZ 1
 
-template <int NR, int NM, int CB>
+template <int NR, int NM, int CB, bool FINE>
 __global__ void __launch_bounds__(ADJ_BX *ADJ_BY *ADJ_BZ)
 adjoint_gather_kernel(const float *__restrict__ sinoI, float *__restrict__ vol, const __grid_constant__ AdjGeom G,
                       const __grid_constant__ ViewChunk V, int q0, int accumulate, size_t sino_cstride,
@@ -182,7 +182,7 @@ adjoint_gather_kernel(const float *__restrict__ sinoI, float *__restrict__ vol, 
                     if (j == 4 && fmaf(lam_hi, invg, -5.5f) <= klo) break;  // k = klo + 5 is past the window
                     ex += gNx; ey += gNy; ez += gv;
                 }
-                if (G.step < 0.5f) {  // finer steps: walk the rest of the window (uniform branch)
+                if (FINE) {  // steps finer than 1/2 voxel: walk the rest of the window
                     const float kend = fmaf(lam_hi, invg, -0.5f);  // samples with k < kend are inside
                     for (float kf = klo + 6.0f; kf < kend; kf += 1.0f) {
                         const float wx = fmaxf(1.0f - fabsf(ex), 0.f);
@@ -295,7 +295,8 @@ static int launch_gather(cbct_geom *g, AdjGeom &G, const float *sinoI, float *vo
         G.split_stride = (size_t)CB * nvox;
         grid.z = nzb * nsplit;
         cbct_prof_begin(g, CBCT_KERNEL_ADJOINT, st);
-        adjoint_gather_kernel<NR, NM, CB><<<grid, block, 0, st>>>(sinoI, partial, G, vc, 0, 0, sstride, nvox, 0);
+        if (G.step < 0.5f) adjoint_gather_kernel<NR, NM, CB, true><<<grid, block, 0, st>>>(sinoI, partial, G, vc, 0, 0, sstride, nvox, 0);
+        else adjoint_gather_kernel<NR, NM, CB, false><<<grid, block, 0, st>>>(sinoI, partial, G, vc, 0, 0, sstride, nvox, 0);
         cbct_prof_end(g, CBCT_KERNEL_ADJOINT, st);
         int rc = cbct_check_launch(g, "adjoint_gather_kernel");
         if (rc) return rc;
@@ -310,8 +311,12 @@ static int launch_gather(cbct_geom *g, AdjGeom &G, const float *sinoI, float *vo
         for (int i = 0; i < n; ++i) vc.cs[i] = make_double2(g->cosphi[q0 + i], g->sinphi[q0 + i]);
         G.nq = n;
         cbct_prof_begin(g, CBCT_KERNEL_ADJOINT, st);
-        adjoint_gather_kernel<NR, NM, CB><<<grid, block, 0, st>>>(sinoI, vol, G, vc, q0, accumulate_first || q0 > 0,
-                                                                  sstride, vstride, vol_z_origin);
+        if (G.step < 0.5f)
+            adjoint_gather_kernel<NR, NM, CB, true><<<grid, block, 0, st>>>(sinoI, vol, G, vc, q0, accumulate_first || q0 > 0,
+                                                                            sstride, vstride, vol_z_origin);
+        else
+            adjoint_gather_kernel<NR, NM, CB, false><<<grid, block, 0, st>>>(sinoI, vol, G, vc, q0, accumulate_first || q0 > 0,
+                                                                             sstride, vstride, vol_z_origin);
         cbct_prof_end(g, CBCT_KERNEL_ADJOINT, st);
         int rc = cbct_check_launch(g, "adjoint_gather_kernel");
         if (rc) return rc;
