@@ -93,8 +93,9 @@ typedef struct cbct_geom_desc {
  * passed to the kernels through constant memory) and returns a handle in
  * *out.  Needs no CUDA device (device workspace is allocated lazily by the
  * first compute call).  Requires sdd > sid, the sphere bounding the
- * zero-extended volume strictly between source and detector plane, positive
- * sizes and pitches, 0 < step_vox <= 1. */
+ * zero-extended volume strictly between source and detector plane (with two
+ * voxels of clearance on the source side), positive sizes and pitches,
+ * 0 < step_vox <= 1. */
 int cbct_geom_create(const cbct_geom_desc *d, cbct_geom **out);
 
 /* Frees the handle, its tables and its device workspace (synchronises the device). */

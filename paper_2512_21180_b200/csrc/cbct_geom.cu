@@ -55,7 +55,8 @@ extern "C" int cbct_geom_create(const cbct_geom_desc *d, cbct_geom **out)
            hz = 0.5 * (d->vol_nz + 1) * d->vox_mm;
     double rc = sqrt(d->vol_cx_mm * d->vol_cx_mm + d->vol_cy_mm * d->vol_cy_mm + d->vol_cz_mm * d->vol_cz_mm);
     double rbound = rc + sqrt(hx * hx + hy * hy + hz * hz);
-    if (!(rbound < d->sid_mm)) return CBCT_ERR_INVALID_ARG;
+    // (two voxels of clearance: the gather adjoint bounds its ray search with U - 1.5 voxels > 0)
+    if (!(rbound + 2.0 * d->vox_mm < d->sid_mm)) return CBCT_ERR_INVALID_ARG;
     // ... and strictly in front of the detector plane, so every in-support
     // sample has t_k < |p - s| (the forward sum stops at the detector).
     if (!(rbound < d->sdd_mm - d->sid_mm)) return CBCT_ERR_INVALID_ARG;
