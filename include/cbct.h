@@ -34,8 +34,11 @@
  *   - Every data pointer may be a DEVICE pointer or a HOST pointer (pinned or
  *     pageable); the library detects which with cudaPointerGetAttributes.
  *     Host buffers are staged through library-owned device workspace inside
- *     the call (copies are enqueued on `cuda_stream`; a call with any pageable
- *     host buffer synchronises the stream before returning).
+ *     the call: without a work-set cap, as a pipeline over blocks of 2 channels
+ *     (H2D copy / kernels / D2H copy on three streams, joined back into
+ *     `cuda_stream` before the call's work ends); with a cap, by z-slabs (A5).
+ *     A call with any pageable host buffer synchronises the stream before
+ *     returning.
  *   - Outputs are OVERWRITTEN, never accumulated into.
  *   - Ownership: the caller owns all data buffers; the library owns the
  *     handle and its device workspace, freed by cbct_geom_destroy.

@@ -88,6 +88,73 @@ static int begin_call(const cbct_geom *gc, const void *vol, const void *sino, in
 // ---------------------------------------------------------------------------
 // A2 + A5
 // ---------------------------------------------------------------------------
+// ---------------------------------------------------------------------------
+// HOST buffers without a work-set cap: the call is cut into blocks of 2 channels that flow through a
+// three-stage pipeline -- H2D copy of block b+1 (one stream), the device implementation on block b (the
+// caller's stream), D2H copy of block b-1 (another stream) -- with two device buffers per side, so the
+// PCIe copies in both directions hide behind the kernels.  `inner(din, dout, c0, nc)` enqueues the
+// device implementation for channels [c0, c0 + nc) on the caller's stream.
+// ---------------------------------------------------------------------------
+template <class Inner>
+static int blocked_call(CallCtx &cx, const float *in, size_t n_in, MemKind kin, float *out, size_t n_out, MemKind kout,
+                        Inner inner)
+{
+    cbct_geom *g = cx.g;
+    cudaStream_t st = cx.st;
+    const int BK = 2, channels = cx.channels;
+    if (!g->h2d_stream) CBCT_CUDA_TRY(cudaStreamCreateWithFlags(&g->h2d_stream, cudaStreamNonBlocking));
+    if (!g->d2h_stream) CBCT_CUDA_TRY(cudaStreamCreateWithFlags(&g->d2h_stream, cudaStreamNonBlocking));
+    for (int i = 0; i < 7; ++i)
+        if (!g->ev_blk[i]) CBCT_CUDA_TRY(cudaEventCreateWithFlags(&g->ev_blk[i], cudaEventDisableTiming));
+    cudaEvent_t *evH = g->ev_blk, *evC = g->ev_blk + 2, *evD = g->ev_blk + 4, ev0 = g->ev_blk[6];
+    int rc;
+    if (kin != MEM_DEVICE) {
+        rc = ensure(&g->ws_blk_in, &g->ws_blk_in_bytes, 2 * BK * n_in * sizeof(float));
+        if (rc) return rc;
+    }
+    if (kout != MEM_DEVICE) {
+        rc = ensure(&g->ws_blk_out, &g->ws_blk_out_bytes, 2 * BK * n_out * sizeof(float));
+        if (rc) return rc;
+    }
+    // the copy streams start after everything already queued on `st`
+    CBCT_CUDA_TRY(cudaEventRecord(ev0, st));
+    CBCT_CUDA_TRY(cudaStreamWaitEvent(g->h2d_stream, ev0, 0));
+    CBCT_CUDA_TRY(cudaStreamWaitEvent(g->d2h_stream, ev0, 0));
+    const int nb = (channels + BK - 1) / BK;
+    for (int b = 0; b < nb; ++b) {
+        const int i = b & 1, c0 = b * BK, nc = channels - c0 < BK ? channels - c0 : BK;
+        const float *din = in + (size_t)c0 * n_in;
+        float *dout = out + (size_t)c0 * n_out;
+        if (kin != MEM_DEVICE) {
+            float *buf = g->ws_blk_in + (size_t)i * BK * n_in;
+            if (b >= 2) CBCT_CUDA_TRY(cudaStreamWaitEvent(g->h2d_stream, evC[i], 0));  // block b-2 consumed
+            CBCT_CUDA_TRY(cudaMemcpyAsync(buf, din, (size_t)nc * n_in * sizeof(float), cudaMemcpyHostToDevice, g->h2d_stream));
+            CBCT_CUDA_TRY(cudaEventRecord(evH[i], g->h2d_stream));
+            CBCT_CUDA_TRY(cudaStreamWaitEvent(st, evH[i], 0));
+            din = buf;
+        }
+        if (kout != MEM_DEVICE) {
+            if (b >= 2) CBCT_CUDA_TRY(cudaStreamWaitEvent(st, evD[i], 0));  // block b-2 copied out
+            dout = g->ws_blk_out + (size_t)i * BK * n_out;
+        }
+        rc = inner(din, dout, c0, nc);
+        if (rc) return rc;
+        CBCT_CUDA_TRY(cudaEventRecord(evC[i], st));
+        if (kout != MEM_DEVICE) {
+            CBCT_CUDA_TRY(cudaStreamWaitEvent(g->d2h_stream, evC[i], 0));
+            CBCT_CUDA_TRY(cudaMemcpyAsync(out + (size_t)c0 * n_out, dout, (size_t)nc * n_out * sizeof(float),
+                                          cudaMemcpyDeviceToHost, g->d2h_stream));
+            CBCT_CUDA_TRY(cudaEventRecord(evD[i], g->d2h_stream));
+        }
+    }
+    if (kout != MEM_DEVICE) {  // join the D2H stream back into `st`
+        CBCT_CUDA_TRY(cudaStreamWaitEvent(st, evD[0], 0));
+        if (nb > 1) CBCT_CUDA_TRY(cudaStreamWaitEvent(st, evD[1], 0));
+    }
+    if (cx.pageable) CBCT_CUDA_TRY(cudaStreamSynchronize(st));
+    return CBCT_OK;
+}
+
 // y != nullptr: sino = P vol - y (the residual of the Landweber term, fused into the epilogue; y is a
 // DEVICE sinogram).  In the slab path the sinogram starts as -y instead of zero.
 static int fp_impl(const cbct_geom *gc, const float *vol, const float *y, float *sino, int32_t channels, void *stream)
@@ -104,6 +171,11 @@ static int fp_impl(const cbct_geom *gc, const float *vol, const float *y, float 
     const int n_slabs = (nz + planes - 1) / planes;
     const int nbuf = n_slabs > 1 ? 2 : 1;
     const bool host_vol = cx.kv != MEM_DEVICE;
+    if ((host_vol || cx.ks != MEM_DEVICE) && g->d.max_workset_bytes == 0)
+        return blocked_call(cx, vol, cx.nvol, cx.kv, sino, cx.nsino, cx.ks,
+                            [&](const float *dv, float *ds, int c0, int nc) {
+                                return fp_impl(gc, dv, y ? y + (size_t)c0 * cx.nsino : nullptr, ds, nc, stream);
+                            });
 
     float *d_sino = sino;
     if (cx.ks != MEM_DEVICE) {
@@ -238,6 +310,11 @@ static int adjoint_impl(const cbct_geom *gc, const float *sino, float *vol, int3
     cbct_geom *g = cx.g;
     cudaStream_t st = cx.st;
     const size_t sino_bytes = cx.nsino * channels * sizeof(float);
+    if ((cx.kv != MEM_DEVICE || cx.ks != MEM_DEVICE) && g->d.max_workset_bytes == 0)
+        return blocked_call(cx, sino, cx.nsino, cx.ks, vol, cx.nvol, cx.kv,
+                            [&](const float *ds, float *dv, int, int nc) {
+                                return adjoint_impl(gc, ds, dv, nc, stream, weighted);
+                            });
 
     const float *d_sino = sino;
     if (cx.ks != MEM_DEVICE) {
@@ -300,6 +377,9 @@ extern "C" int cbct_bp_fdk(const cbct_geom *gc, const float *sino, float *vol, i
     if (rc) return rc;
     cbct_geom *g = cx.g;
     cudaStream_t st = cx.st;
+    if ((cx.kv != MEM_DEVICE || cx.ks != MEM_DEVICE) && g->d.max_workset_bytes == 0)
+        return blocked_call(cx, sino, cx.nsino, cx.ks, vol, cx.nvol, cx.kv,
+                            [&](const float *ds, float *dv, int, int nc) { return cbct_bp_fdk(gc, ds, dv, nc, stream); });
 
     // zero-bordered, rotation-interleaved copy of the sinogram (cbct_fdk.cu)
     const int pu = cbct_padded_sino_pitch(g), pv = cbct_padded_sino_rows(g);

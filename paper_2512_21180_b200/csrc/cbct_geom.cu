@@ -105,7 +105,7 @@ static void prof_clear(cbct_geom *g);
 extern "C" int cbct_geom_destroy(cbct_geom *g)
 {
     if (!g) return CBCT_ERR_INVALID_ARG;
-    if (g->ws_vol || g->ws_sino || g->ws_sino2 || g->ws_stage || g->copy_stream || g->d_filter_tab) {
+    if (g->ws_vol || g->ws_sino || g->ws_sino2 || g->ws_stage || g->copy_stream || g->d_filter_tab || g->h2d_stream) {
         cudaDeviceSynchronize();
         cudaFree(g->ws_vol);
         cudaFree(g->ws_sino);
@@ -116,6 +116,12 @@ extern "C" int cbct_geom_destroy(cbct_geom *g)
             if (g->ev[i]) cudaEventDestroy(g->ev[i]);
         prof_clear(g);
         if (g->copy_stream) cudaStreamDestroy(g->copy_stream);
+        cudaFree(g->ws_blk_in);
+        cudaFree(g->ws_blk_out);
+        for (int i = 0; i < 7; ++i)
+            if (g->ev_blk[i]) cudaEventDestroy(g->ev_blk[i]);
+        if (g->h2d_stream) cudaStreamDestroy(g->h2d_stream);
+        if (g->d2h_stream) cudaStreamDestroy(g->d2h_stream);
     }
     delete g;
     return CBCT_OK;

@@ -63,6 +63,11 @@ struct cbct_geom {
     float *ws_stage = nullptr; size_t ws_stage_bytes = 0;  // raw planes of a host volume on their way to the pack kernel
     cudaStream_t copy_stream = nullptr;
     cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
+    // channel-block pipeline for HOST buffers (cbct_api.cu): H2D and D2H streams, double-buffered blocks
+    cudaStream_t h2d_stream = nullptr, d2h_stream = nullptr;
+    cudaEvent_t ev_blk[7] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+    float *ws_blk_in = nullptr;  size_t ws_blk_in_bytes = 0;
+    float *ws_blk_out = nullptr; size_t ws_blk_out_bytes = 0;
     uint64_t launches = 0;
     int64_t sample_count = -1;
     float *d_filter_tab = nullptr;  // FDK front-end tables (cbct_fdk_filter.cu), built on first use
