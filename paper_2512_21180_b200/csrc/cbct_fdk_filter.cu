@@ -56,7 +56,6 @@ fdk_filter_kernel(const float *__restrict__ in, float *__restrict__ out, const f
 // (even / odd columns).  For a set with outputs j0 + 2i the inputs of tap n+2 are those of tap n shifted by one
 // output (c[j0+2i-(n+2)] = c[j0+2(i-1)-n]), so each step loads only one new value on each side and reuses the
 // other three from registers: 2 LDS + 1 broadcast tap per 8 multiply-adds instead of 3 per 2.
-template <int DUMMY>
 __global__ void __launch_bounds__(256)
 fdk_filter8_kernel(const float *__restrict__ in, float *__restrict__ out, const float *__restrict__ tab_w,
                    const float *__restrict__ tab_h, int nu, int nv, size_t n_rows, float u0, float du, float v0,
@@ -237,8 +236,8 @@ extern "C" int cbct_fdk_filter(const cbct_geom *gc, const float *sino_in, float 
         const size_t smem8 = ((size_t)nu + (size_t)rpc * (span + span / 32 + 1)) * sizeof(float);
         const size_t want = (n_rows + rpc - 1) / rpc;
         const unsigned grid8 = (unsigned)(want < 148u * 8u ? want : 148u * 8u);
-        fdk_filter8_kernel<0><<<grid8, dim3(tpr, rpc), smem8, st>>>(sino_in, sino_out, tw, g->d_filter_tab + 2 * (size_t)nu,
-                                                                  nu, d.det_nv, n_rows, fu0, (float)d.det_du_mm, fv0,
+        fdk_filter8_kernel<<<grid8, dim3(tpr, rpc), smem8, st>>>(sino_in, sino_out, tw, g->d_filter_tab + 2 * (size_t)nu, nu,
+                                                               d.det_nv, n_rows, fu0, (float)d.det_du_mm, fv0,
                                                                   (float)d.det_dv_mm, (float)d.sdd_mm);
         return cbct_check_launch(g, "fdk_filter8_kernel");
     }
