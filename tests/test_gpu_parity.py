@@ -257,7 +257,7 @@ def test_errors_are_loud(cbct):
 @pytest.mark.parametrize("name", ["pyramid_64", "pyramid_128", "pyramid_256"])
 def test_config3_pyramid_sampled(cbct, oracle_mod, name):
     """Config 3 at full size, in the launch configuration bench.py times:
-    2000 sampled rays, 48 sampled adjoint voxels, 2000 sampled FDK voxels, each
+    2000 sampled rays, 256 sampled adjoint voxels, 2000 sampled FDK voxels, each
     computed one by one by the oracle; plus the fp32 adjoint identity."""
     cfg = synth.CONFIGS[name]
     kw = synth.geom_kwargs(cfg)
@@ -271,7 +271,7 @@ def test_config3_pyramid_sampled(cbct, oracle_mod, name):
     floor = 1e-3 * float(np.max(np.abs(r)))
     assert np.max(np.abs(gsel - r) / np.maximum(np.abs(r), floor)) <= 1e-4
     Aty = run_adj(cbct, kw, sino)
-    vidx = synth.sample_indices(12, vol[0].size, 48)
+    vidx = synth.sample_indices(12, vol[0].size, 256)
     r = oracle_mod.bp_adjoint_voxels(og, sino.astype(np.float64), vidx)
     assert rel_l2(Aty.reshape(1, -1)[:, vidx], r) <= 1e-4
     lhs, rhs = float(np.sum(Ax * sino)), float(np.sum(vol.astype(np.float64) * Aty))
@@ -316,7 +316,7 @@ def test_config4_multichannel_sampled(cbct, oracle_mod):
     Ax, Aty, F = run_fp(cbct, kw, vol), run_adj(cbct, kw, sino), run_fdk(cbct, kw, sino)
     for c in (0, 1, 7):
         _sampled_checks(oracle_mod, og, vol[c], sino[c], Ax[c], Aty[c], F[c], (41 + c, 51 + c, 61 + c),
-                        n_rays=800, n_adj=16, n_fdk=800)
+                        n_rays=800, n_adj=64, n_fdk=800)
     # channel independence at full size: channel 3 alone gives the same bits as channel 3 of the batch
     one = run_fp(cbct, kw, vol[3:4])
     assert np.array_equal(one[0], Ax[3])
@@ -346,7 +346,7 @@ def test_config5_large_streamed_sampled(cbct, oracle_mod):
     Ax_h, sino_h, vol_h = Ax.cpu().numpy(), sino.cpu().numpy(), vol.numpy()
     for c in (0, 1):
         _sampled_checks(oracle_mod, og, vol_h[c], sino_h[c], Ax_h[c], Aty[c], F[c], (71 + c, 81 + c, 91 + c),
-                        n_rays=1000, n_adj=12, n_fdk=1000)
+                        n_rays=1000, n_adj=48, n_fdk=1000)
     lhs = float(np.sum(Ax_h[0].astype(np.float64) * sino_h[0]))
     rhs = float(np.sum(vol_h[0].astype(np.float64) * Aty[0]))
     assert abs(lhs - rhs) / abs(lhs) <= 1e-5, (lhs, rhs)
