@@ -334,8 +334,16 @@ static int launch_gather_channels(cbct_geom *g, AdjGeom &G, const float *sinoI, 
         int left = channels - c, rc;
         const float *s = sinoI + c * sstride;
         float *v = vol + c * vstride;
-        // 2 channels per thread: 4 needs 128 registers and measured slower (158 vs 143 ms at C = 8)
-        if (left >= 2 && NR * NM <= 8) { rc = launch_gather<NR, NM, 2>(g, G, s, v, 0, sstride, vstride, vol_z_origin, partial, nsplit, st); c += 2; }
+        // One weight evaluation feeds NR * NM * CB accumulators; 16 is the sweet spot (with all symmetries, 2
+        // channels: 4 need 128 registers and measured slower, 158 vs 143 ms at C = 8).  Geometries with fewer
+        // symmetries (irregular view angles, off-centre grids) make it up with more channels per thread.
+        if constexpr (NR * NM <= 2) {
+            if (left >= 8) { rc = launch_gather<NR, NM, 8>(g, G, s, v, 0, sstride, vstride, vol_z_origin, partial, nsplit, st); c += 8; if (rc) return rc; continue; }
+        }
+        if constexpr (NR * NM <= 4) {
+            if (left >= 4) { rc = launch_gather<NR, NM, 4>(g, G, s, v, 0, sstride, vstride, vol_z_origin, partial, nsplit, st); c += 4; if (rc) return rc; continue; }
+        }
+        if (left >= 2) { rc = launch_gather<NR, NM, 2>(g, G, s, v, 0, sstride, vstride, vol_z_origin, partial, nsplit, st); c += 2; }
         else { rc = launch_gather<NR, NM, 1>(g, G, s, v, 0, sstride, vstride, vol_z_origin, partial, nsplit, st); c += 1; }
         if (rc) return rc;
     }
@@ -360,7 +368,7 @@ int cbct_adjoint_view_splits(const cbct_geom *g)
     return s < 1 ? 1 : (int)s;
 }
 
-// `partial` (nsplit > 1 only): workspace of nsplit * 2 * nx * ny * nz floats; used when the launch covers the
+// `partial` (nsplit > 1 only): workspace of nsplit * 8 * nx * ny * nz floats; used when the launch covers the
 // whole grid (zs0 = 0, zs1 = nz, vol_z_origin = 0).
 int cbct_launch_adjoint(cbct_geom *g, const float *sino_src, float *vol, int channels, int zs0, int zs1,
                         size_t vol_channel_stride, int vol_z_origin, float *partial, int nsplit, cudaStream_t st)

@@ -344,7 +344,7 @@ static int adjoint_impl(const cbct_geom *gc, const float *sino, float *vol, int3
     int nsplit = cx.kv == MEM_DEVICE ? cbct_adjoint_view_splits(g) : 1;
     float *partial = nullptr;
     if (nsplit > 1) {
-        rc = ensure(&g->ws_vol, &g->ws_vol_bytes, (size_t)nsplit * 2 * cx.nvol * sizeof(float));
+        rc = ensure(&g->ws_vol, &g->ws_vol_bytes, (size_t)nsplit * 8 * cx.nvol * sizeof(float));
         if (rc) return rc;
         partial = g->ws_vol;
     }
