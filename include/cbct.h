@@ -190,6 +190,23 @@ int cbct_geom_profile(cbct_geom *g, int enable);
 int cbct_geom_profile_read(cbct_geom *g, int kernel, double *ms_total, uint64_t *launches);
 
 /* Static description of a status code. */
+/* NEXT-4: pointwise steps of the polychromatic primary model, DEVICE pointers.
+ * cbct_water_bone, Eq. (3)-(4): rho_w[i], rho_b[i] from the modified CT number rho_hat[i] = 0.001 HU + 1
+ *   rho_w = 0 (r < tau0), r (r < tau1), tau1 (tau2 - r)/(tau2 - tau1) (r < tau2), 0 otherwise;
+ *   rho_b = 0 (r < tau1), kappa_b tau2 (r - tau1)/(tau2 - tau1) (r < tau2), kappa_b r otherwise.
+ * The paper's constants are tau1 = 1.2, tau2 = 1.6, kappa_b = 0.409; it does not print tau0 (reading R23: the
+ * caller's, 0 keeps all soft tissue).  n elements each; outputs overwritten; needs tau0 <= tau1 < tau2.
+ * cbct_polychromatic_primary, Eq. (6) without the Poisson draw (its mean):
+ *   out[q][p] = sum_e resp[e] i0[e][p] exp(-(mu_w[e] pw[q][p] + mu_b[e] pb[q][p])),
+ * pw, pb = cbct_fp of rho_w, rho_b ([n_views][n_pix], mm), i0: [n_bins][n_pix] unattenuated counts per energy bin and
+ * detector element, mu_w / mu_b / resp: HOST arrays of n_bins (<= 32) doubles (attenuation per unit relative
+ * density in 1/mm; detector response), read before the call returns. */
+int cbct_water_bone(const float *rho_hat, float *rho_w, float *rho_b, int64_t n, double tau0, double tau1, double tau2,
+                    double kappa_b, void *cuda_stream);
+int cbct_polychromatic_primary(const float *pw, const float *pb, const float *i0, const double *mu_w,
+                               const double *mu_b, const double *resp, int32_t n_bins, int64_t n_views, int64_t n_pix,
+                               float *out, void *cuda_stream);
+
 const char *cbct_status_string(int status);
 
 /* Text of the last CUDA error seen by the calling thread ("" if none). */

@@ -6,6 +6,8 @@ Only ``tests/``, ``__graft_entry__.smoke()`` and ``bench.py``'s
 imports nothing from ``paper_2512_21180_b200`` and shares no code with the
 CUDA path.  Definitions: PAPER.md:85-89 (Eq. 5), PAPER.md:61 (geometry),
 PAPER.md:157/181/397 (FDK); discretisation readings R1-R11 in DESIGN.md s.3.
+The NEXT rows of SURVEY.md s.8(f) (FDK front end, FoV tensor, resampling, water-bone /
+polychromatic mean) are plain numpy below, each citing its passage; pins P13-P17.
 """
 from __future__ import annotations
 
@@ -325,3 +327,33 @@ def proj_down(p, factor: int) -> np.ndarray:
     nv, nu = p.shape[-2:]
     assert nv % f == 0 and nu % f == 0
     return p.reshape(p.shape[:-2] + (nv // f, f, nu // f, f)).mean(axis=(-3, -1))
+
+
+# ---------------------------------------------------------------------------
+# NEXT-4: water-bone decomposition (Eq. 3-4) and the noise-free polychromatic primary (Eq. 6)
+# ---------------------------------------------------------------------------
+def detector_response(energy_kev) -> np.ndarray:
+    """resp(e): piecewise linear through r_20 = 5, r_60 = 20, r_120 = 10 (keV)."""
+    return np.interp(np.asarray(energy_kev, dtype=np.float64), [20.0, 60.0, 120.0], [5.0, 20.0, 10.0])
+
+
+def water_bone(rho_hat, tau0: float = 0.0, tau1: float = 1.2, tau2: float = 1.6, kappa_b: float = 0.409):
+    """Eq. (3)-(4): relative water / bone densities as functions of the modified CT number
+    rho_hat = 0.001 HU + 1.  tau_1, tau_2, kappa_b are the paper's constants; tau_0 (the lower cut of the water
+    branch) is named but not given a value in the paper -- reading R23: a caller parameter, default 0."""
+    r = np.asarray(rho_hat, dtype=np.float64)
+    rw = np.where(r < tau0, 0.0, np.where(r < tau1, r, np.where(r < tau2, tau1 * (tau2 - r) / (tau2 - tau1), 0.0)))
+    rb = np.where(r < tau1, 0.0, np.where(r < tau2, kappa_b * tau2 * (r - tau1) / (tau2 - tau1), kappa_b * r))
+    return rw, rb
+
+
+def polychromatic_primary(pw, pb, i0, mu_w, mu_b, resp) -> np.ndarray:
+    """Noise-free mean of Eq. (6): sum_e resp(e) I_{0,e}(sigma) exp(-(mu_w(e) P rho_w + mu_b(e) P rho_b))
+    (the projector is linear, so P(mu~_e^w + mu~_e^b) = mu_w(e) P(rho_w) + mu_b(e) P(rho_b)).
+    pw, pb: [n_views, nv, nu] line integrals of rho_w, rho_b (mm); i0: [n_bins, nv, nu] unattenuated counts per bin
+    and detector element; mu_w, mu_b: [n_bins] attenuation per unit relative density (1/mm); resp: [n_bins]."""
+    pw, pb, i0 = (np.asarray(a, dtype=np.float64) for a in (pw, pb, i0))
+    out = np.zeros_like(pw)
+    for e in range(len(resp)):
+        out += resp[e] * i0[e][None] * np.exp(-(mu_w[e] * pw + mu_b[e] * pb))
+    return out

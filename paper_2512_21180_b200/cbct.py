@@ -24,6 +24,7 @@ EXPORTS = (
     "cbct_fdk_filter", "cbct_redundancy_weight", "cbct_geom_redundancy_weights",
     "cbct_fp_residual", "cbct_bp_adjoint_weighted",
     "cbct_fov", "cbct_downsample", "cbct_upsample", "cbct_proj_down",
+    "cbct_water_bone", "cbct_polychromatic_primary",
     "cbct_status_string", "cbct_last_cuda_error",
 )
 
@@ -83,6 +84,10 @@ def load_library() -> ctypes.CDLL:
     L.cbct_downsample.argtypes = [vp, vp, i64, i32, i32, i32, i32, vp]
     L.cbct_upsample.argtypes = [vp, vp, i64, i32, i32, i32, i32, vp]
     L.cbct_proj_down.argtypes = [vp, vp, i64, i32, i32, i32, i32, vp]
+    f64 = ctypes.c_double
+    L.cbct_water_bone.argtypes = [vp, vp, vp, i64, f64, f64, f64, f64, vp]
+    dp = ctypes.POINTER(ctypes.c_double)
+    L.cbct_polychromatic_primary.argtypes = [vp, vp, vp, dp, dp, dp, i32, i64, i64, vp, vp]
     L.cbct_status_string.argtypes = [ctypes.c_int]
     L.cbct_status_string.restype = ctypes.c_char_p
     L.cbct_last_cuda_error.restype = ctypes.c_char_p
@@ -286,3 +291,27 @@ def proj_down(sino_in, sino_out, factor: int, stream=None):
     po = _ptr_and_keep(sino_out, o * (-(-nviews // factor)) * (nv // factor) * (nu // factor))
     _check(load_library().cbct_proj_down(pi, po, o, nviews, nv, nu, factor, _stream_handle(stream)))
     return sino_out
+
+
+def water_bone(rho_hat, rho_w, rho_b, tau0: float = 0.0, tau1: float = 1.2, tau2: float = 1.6,
+               kappa_b: float = 0.409, stream=None):
+    """cbct_water_bone: Eq. (3)-(4) water / bone densities of a modified-CT-number array (any shape)."""
+    n = int(np.prod(rho_hat.shape))
+    pr, pw, pb = (_ptr_and_keep(t, n) for t in (rho_hat, rho_w, rho_b))
+    _check(load_library().cbct_water_bone(pr, pw, pb, n, tau0, tau1, tau2, kappa_b, _stream_handle(stream)))
+    return rho_w, rho_b
+
+
+def polychromatic_primary(pw, pb, i0, mu_w, mu_b, resp, out, stream=None):
+    """cbct_polychromatic_primary: noise-free Eq. (6); pw, pb, out [n_views, nv, nu], i0 [n_bins, nv, nu]."""
+    n_bins = len(resp)
+    if len(mu_w) != n_bins or len(mu_b) != n_bins or i0.shape[0] != n_bins:
+        raise CbctError("mu_w, mu_b, resp and i0 must agree on the number of energy bins")
+    n_views = int(pw.shape[0])
+    n_pix = int(np.prod(pw.shape[1:]))
+    pa, pb_, po = (_ptr_and_keep(t, n_views * n_pix) for t in (pw, pb, out))
+    pi = _ptr_and_keep(i0, n_bins * n_pix)
+    arr = [(ctypes.c_double * n_bins)(*[float(x) for x in t]) for t in (mu_w, mu_b, resp)]
+    _check(load_library().cbct_polychromatic_primary(pa, pb_, pi, arr[0], arr[1], arr[2], n_bins, n_views, n_pix, po,
+                                                     _stream_handle(stream)))
+    return out

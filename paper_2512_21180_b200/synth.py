@@ -143,3 +143,23 @@ def sample_indices(seed: int, total: int, count: int) -> np.ndarray:
     """Seeded sorted unique flat indices for sampled parity at full sizes."""
     rng = np.random.default_rng(seed)
     return np.unique(rng.integers(0, total, size=count, dtype=np.int64))
+
+
+def spectrum_tables(nv: int, nu: int, n_bins: int = 10, seed: int = 5):
+    """Made-up inputs for the polychromatic primary (NEXT-4): bin centres 25, 35, ... keV (PAPER.md:61 names ten
+    bins centred 25..115 keV), attenuation per unit relative density and mm for "water" and "bone" as smooth
+    decreasing power laws of the energy (NOT xraylib's tables, which are not in this container), and per-bin
+    unattenuated counts i0[e, v, u] = spectrum weight x a smooth bow-tie-like beam profile x (1 + 2% seeded ripple).
+    Returns (energies_kev, mu_w, mu_b, i0 fp32)."""
+    e = 25.0 + 10.0 * np.arange(n_bins)
+    mu_w = 0.016 + 0.011 * (60.0 / e) ** 2.7
+    mu_b = 0.025 + 0.040 * (60.0 / e) ** 3.0
+    spec = np.exp(-0.5 * ((e - 60.0) / 28.0) ** 2)
+    spec *= 2.0e4 / spec.sum()
+    u = (np.arange(nu) + 0.5) / nu - 0.5
+    v = (np.arange(nv) + 0.5) / nv - 0.5
+    profile = (0.35 + 0.65 * np.cos(np.pi * u) ** 2)[None, :] * (1.0 - 0.2 * v[:, None] ** 2)
+    rng = np.random.default_rng(seed)
+    ripple = 1.0 + 0.02 * rng.standard_normal((n_bins, nv, nu))
+    i0 = (spec[:, None, None] * profile[None] * ripple).astype(np.float32)
+    return e, mu_w, mu_b, i0

@@ -481,6 +481,72 @@ def test_next2_resampling(cbct, oracle_mod):
         cbct.downsample(dev(z), torch.empty((3, 2, 4, 6), device="cuda"), 3)
 
 
+def test_next4_water_bone(cbct, oracle_mod):
+    """NEXT-4: Eq. 3-4 against the oracle, with the paper's constants and a tau_0 that fp32 holds exactly; ragged
+    length, an unaligned view (scalar path) and the empty input.  fp32 arithmetic on O(1) values: 1e-6 absolute."""
+    rng = np.random.default_rng(41)
+    r = (rng.random(4099) * 2.6 - 0.1).astype(np.float32)
+    r[:6] = np.float32([1.2, 1.6, 0.125, 0.0, 1.4, 2.0])
+    for lo, tau0 in ((0, 0.0), (0, 0.125), (1, 0.125)):
+        src = dev(r)[lo:]
+        w, b = torch.full_like(src, float("nan")), torch.full_like(src, float("nan"))
+        cbct.water_bone(src, w, b, tau0=tau0)
+        ww, wb = oracle_mod.water_bone(r[lo:].astype(np.float64), tau0=tau0)
+        assert np.max(np.abs(w.cpu().numpy() - ww)) <= 1e-6 and np.max(np.abs(b.cpu().numpy() - wb)) <= 1e-6
+    e = torch.empty(0, device="cuda")
+    cbct.water_bone(e, e.clone(), e.clone())
+    with pytest.raises(cbct.CbctError):
+        cbct.water_bone(dev(r), dev(r), dev(r), tau1=1.7)
+
+
+@pytest.mark.parametrize("shape", [(7, 12, 20), (3, 5, 7), (70, 16, 24)])
+def test_next4_polychromatic_primary(cbct, oracle_mod, shape):
+    """NEXT-4: noise-free Eq. 6 on given line integrals.  Exponents reach ~20; their fp32 rounding (coefficient,
+    product, sum: ~3 x 2^-24 x 20) and exp2f's 2 ulp bound the relative error by ~5e-6 per term: 1e-5."""
+    nq, nv, nu = shape
+    rng = np.random.default_rng(43)
+    pw = (rng.random(shape) * 420.0).astype(np.float32)
+    pb = (rng.random(shape) * 60.0).astype(np.float32)
+    en, mu_w, mu_b, i0 = synth.spectrum_tables(nv, nu)
+    resp = oracle_mod.detector_response(en)
+    out = torch.full(shape, float("nan"), device="cuda")
+    cbct.polychromatic_primary(dev(pw), dev(pb), dev(i0), mu_w, mu_b, resp, out)
+    want = oracle_mod.polychromatic_primary(pw, pb, i0, mu_w, mu_b, resp)
+    assert np.max(np.abs(out.cpu().numpy() - want) / want) <= 1e-5
+    one = torch.empty(shape, device="cuda")
+    cbct.polychromatic_primary(dev(pw), dev(pb), dev(i0[3:4]), mu_w[3:4], mu_b[3:4], resp[3:4], one)
+    beer = resp[3] * i0[3].astype(np.float64) * np.exp(-(mu_w[3] * pw.astype(np.float64) + mu_b[3] * pb.astype(np.float64)))
+    assert np.max(np.abs(one.cpu().numpy() - beer) / beer) <= 1e-5
+    with pytest.raises(cbct.CbctError):
+        cbct.polychromatic_primary(dev(pw), dev(pb), dev(i0), mu_w[:4], mu_b, resp, out)
+
+
+def test_next4_chain(cbct, oracle_mod):
+    """NEXT-4 end to end: CT numbers -> (rho_w, rho_b) -> two-channel cbct_fp -> detector signal, each step in the
+    CUDA library, against the same chain in the oracle.  The projector's error (R16: <= 1e-5 of the line integral
+    scale, ~130 mm here) enters the exponent times mu <= 0.2 / mm: relative 3e-4 at most, 1e-4 expected."""
+    cfg = synth.CONFIGS["tiny"]
+    kw = synth.geom_kwargs(cfg)
+    g = cbct.Geometry(**kw)
+    og = oracle_mod.Geom(**kw)
+    ph = synth.make_volume(cfg, 1)[0]
+    rho = np.where(ph > 0, 1.0 + 0.9 * ph / ph.max(), 0.0).astype(np.float32)  # tissue 1..1.9 in air
+    d_rho = dev(rho)
+    wb = torch.empty((2,) + tuple(rho.shape), device="cuda")
+    cbct.water_bone(d_rho, wb[0], wb[1])
+    sino = torch.empty((2,) + tuple(g.sino_shape), device="cuda")
+    g.fp(wb, sino, channels=2)
+    en, mu_w, mu_b, i0 = synth.spectrum_tables(kw["det_nv"], kw["det_nu"])
+    resp = oracle_mod.detector_response(en)
+    out = torch.empty(g.sino_shape, device="cuda")
+    cbct.polychromatic_primary(sino[0], sino[1], dev(i0), mu_w, mu_b, resp, out)
+    ow, ob = oracle_mod.water_bone(rho.astype(np.float64))
+    assert ob.max() > 0 and ow.max() > 0
+    want = oracle_mod.polychromatic_primary(oracle_mod.fp(og, ow)[0], oracle_mod.fp(og, ob)[0], i0, mu_w, mu_b, resp)
+    rel = np.abs(out.cpu().numpy() - want) / want
+    assert rel.max() <= 3e-4 and np.sqrt(np.mean(rel ** 2)) <= 3e-5
+
+
 @pytest.mark.parametrize("over,cap", [(dict(), 0), (dict(n_views=10, vol_nx=30, det_off_u_mm=20.0), 0),
                                       (dict(n_views=7, det_off_u_mm=-15.0), 0), (dict(vol_nz=40, n_views=12, det_off_u_mm=15.0), 2500000)])
 def test_next3_fused_residual_and_weighted_adjoint(cbct, oracle_mod, over, cap):

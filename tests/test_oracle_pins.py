@@ -374,3 +374,28 @@ def test_p16_resampling_definitions(oracle_mod):
     pd = o.proj_down(p, 2)
     assert pd.shape == (3, 4, 2, 3)
     assert pd[2, 1, 1, 2] == pytest.approx(p[2, 2, 2:4, 4:6].sum() / 4.0, abs=1e-15)
+
+
+def test_p17_water_bone_and_polychromatic(oracle_mod):
+    """P17 (NEXT-4): the paper's printed constants -- resp(20, 60, 120 keV) = 5, 20, 10 and linear between;
+    Eq. 3-4 are continuous at tau_1 and tau_2 with the printed values (water: tau_1 at tau_1, 0 at tau_2; bone:
+    0 at tau_1, kappa_b tau_2 at tau_2), water = rho_hat for soft tissue, bone = kappa_b rho_hat above tau_2;
+    one energy bin reduces Eq. 6 to Beer-Lambert; bins add."""
+    o = oracle_mod
+    assert list(o.detector_response([20, 60, 120])) == [5.0, 20.0, 10.0]
+    assert o.detector_response(25.0) == pytest.approx(5.0 + 15.0 * 5.0 / 40.0) and o.detector_response(115.0) == pytest.approx(10.0 + 10.0 * 5.0 / 60.0)
+    eps = 1e-12
+    rw, rb = o.water_bone(np.array([0.5, 1.0, 1.2 - eps, 1.2, 1.4, 1.6 - eps, 1.6, 2.0]))
+    assert rw[1] == 1.0 and rw[0] == 0.5 and rb[0] == rb[1] == 0.0
+    assert rw[2] == pytest.approx(1.2) and rw[3] == pytest.approx(1.2) and rb[3] == 0.0
+    assert rw[4] == pytest.approx(1.2 * 0.2 / 0.4) and rb[4] == pytest.approx(0.409 * 1.6 * 0.2 / 0.4)
+    assert rw[5] == pytest.approx(0.0, abs=1e-10) and rw[6] == 0.0
+    assert rb[5] == pytest.approx(0.409 * 1.6) and rb[6] == pytest.approx(0.409 * 1.6) and rb[7] == pytest.approx(0.409 * 2.0)
+    assert o.water_bone(np.array([0.05]), tau0=0.1)[0][0] == 0.0
+    rng = np.random.default_rng(2)
+    pw, pb = rng.random((3, 4, 5)) * 300, rng.random((3, 4, 5)) * 40
+    i0 = rng.random((2, 4, 5)) * 1e4
+    one = o.polychromatic_primary(pw, pb, i0[:1], [0.02], [0.05], [7.0])
+    assert np.allclose(one, 7.0 * i0[0] * np.exp(-(0.02 * pw + 0.05 * pb)), rtol=1e-15)
+    two = o.polychromatic_primary(pw, pb, i0, [0.02, 0.015], [0.05, 0.03], [7.0, 3.0])
+    assert np.allclose(two, one + o.polychromatic_primary(pw, pb, i0[1:], [0.015], [0.03], [3.0]), rtol=1e-15)
