@@ -89,7 +89,7 @@ static int begin_call(const cbct_geom *gc, const void *vol, const void *sino, in
 // A2 + A5
 // ---------------------------------------------------------------------------
 // ---------------------------------------------------------------------------
-// HOST buffers without a work-set cap: the call is cut into blocks of 2 channels that flow through a
+// HOST buffers without a work-set cap: the call is cut into blocks of 2 channels (4 for the forward projector) that flow through a
 // three-stage pipeline -- H2D copy of block b+1 (one stream), the device implementation on block b (the
 // caller's stream), D2H copy of block b-1 (another stream) -- with two device buffers per side, so the
 // PCIe copies in both directions hide behind the kernels.  `inner(din, dout, c0, nc)` enqueues the
@@ -97,11 +97,11 @@ static int begin_call(const cbct_geom *gc, const void *vol, const void *sino, in
 // ---------------------------------------------------------------------------
 template <class Inner>
 static int blocked_call(CallCtx &cx, const float *in, size_t n_in, MemKind kin, float *out, size_t n_out, MemKind kout,
-                        Inner inner)
+                        Inner inner, int BK = 2)
 {
     cbct_geom *g = cx.g;
     cudaStream_t st = cx.st;
-    const int BK = 2, channels = cx.channels;
+    const int channels = cx.channels;
     if (!g->h2d_stream) CBCT_CUDA_TRY(cudaStreamCreateWithFlags(&g->h2d_stream, cudaStreamNonBlocking));
     if (!g->d2h_stream) CBCT_CUDA_TRY(cudaStreamCreateWithFlags(&g->d2h_stream, cudaStreamNonBlocking));
     for (int i = 0; i < 7; ++i)
@@ -175,7 +175,8 @@ static int fp_impl(const cbct_geom *gc, const float *vol, const float *y, float 
         return blocked_call(cx, vol, cx.nvol, cx.kv, sino, cx.nsino, cx.ks,
                             [&](const float *dv, float *ds, int c0, int nc) {
                                 return fp_impl(gc, dv, y ? y + (size_t)c0 * cx.nsino : nullptr, ds, nc, stream);
-                            });
+                            },
+                            channels >= 4 ? 4 : 2);  // blocks of 4 channels take the channel-interleaved kernel
 
     float *d_sino = sino;
     if (cx.ks != MEM_DEVICE) {

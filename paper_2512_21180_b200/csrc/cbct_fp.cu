@@ -61,6 +61,47 @@ pack_volume_kernel(const float *__restrict__ src, float4 *__restrict__ dst, cons
 }
 
 // ---------------------------------------------------------------------------
+// channel-interleaved layout for groups of 4 channels: cell (jz, jy, jx) holds the voxel's value in the 4
+// channels, float4( v_0, v_1, v_2, v_3 )[jz][jy][jx].  One trilinear sample of 4 channels is then 8 LDG.128 (as
+// many as with 4 quad-packed volumes) but every voxel is stored once instead of four times, so the cells a CTA's
+// beam pulls into L1 are a quarter of the bytes (the quad layout spends 1.7 of its 6.8 data-stage cycles per load
+// on those fills, profiles/r1_final.md).  Rows are not rotated but SKEWED: row (jy, jz) starts
+// (CBCT_SWIZZLE_Y jy + CBCT_SWIZZLE_Z jz) mod 8 cells into a pitch of px + 8, which gives cell jx the same
+// 16-byte line position (jx + 6 jy + 4 jz) mod 8 as the rotation does and keeps jx + 1 one cell further.
+// ---------------------------------------------------------------------------
+#define CBCT_ROW_SKEW 8
+__host__ __device__ __forceinline__ size_t cbct_packed4_cells(const RayGeom &r)
+{
+    return (size_t)(r.px + CBCT_ROW_SKEW) * r.py * r.pz;
+}
+
+// src: 4 consecutive channels [nz_src][ny][nx] each; dst: one channel-interleaved slab
+__global__ void __launch_bounds__(256)
+pack_volume4_kernel(const float *__restrict__ src, float4 *__restrict__ dst, const __grid_constant__ RayGeom G,
+                    size_t src_cstride, int src_z_origin, size_t group_src_stride, size_t group_dst_stride)
+{
+    const float *s = src + (size_t)blockIdx.z * group_src_stride;
+    float4 *d = dst + (size_t)blockIdx.z * group_dst_stride;
+    const int pitch = G.px + CBCT_ROW_SKEW;
+    const int pos = blockIdx.x * blockDim.x + threadIdx.x;
+    if (pos >= pitch) return;
+    for (int row = blockIdx.y; row < G.py * G.pz; row += gridDim.y) {
+        const int jy = row % G.py, jz = row / G.py;
+        const int x = pos - ((CBCT_SWIZZLE_Y * jy + CBCT_SWIZZLE_Z * jz) & 7) - CBCT_PAD;
+        const int y = jy - CBCT_PAD, z = jz - CBCT_PAD + G.z0;
+        float4 q = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (x >= 0 && x < G.nx && y >= 0 && y < G.ny && z >= G.z0 && z < G.z1) {
+            const float *p = s + ((size_t)(z - src_z_origin) * G.ny + y) * G.nx + x;
+            q.x = __ldg(p);
+            q.y = __ldg(p + src_cstride);
+            q.z = __ldg(p + 2 * src_cstride);
+            q.w = __ldg(p + 3 * src_cstride);
+        }
+        d[(size_t)row * pitch + pos] = q;
+    }
+}
+
+// ---------------------------------------------------------------------------
 // forward kernel
 // ---------------------------------------------------------------------------
 #define FP_CTA_U 16
@@ -155,6 +196,76 @@ fp_kernel(const float4 *__restrict__ packed, float *__restrict__ sino, const __g
 }
 
 
+// 4 channels per thread from the channel-interleaved layout; otherwise as fp_kernel.
+struct Acc4 { float a0, a1, a2, a3; };
+
+__device__ __forceinline__ void fp4_sample(const float4 *__restrict__ packed, const Ray &r, float kf, unsigned py,
+                                           unsigned pitch, unsigned plane, unsigned kfold, Acc4 &A)
+{
+    const float yx = fmaf(kf, r.dx, r.ax) + CBCT_MAGIC;
+    const float yy = fmaf(kf, r.dy, r.ay) + CBCT_MAGIC;
+    const float yz = fmaf(kf, r.dz, r.az) + CBCT_MAGIC;
+    const float fx = fmaf(kf, r.dx, r.bx - (yx - CBCT_MAGIC));
+    const float fy = fmaf(kf, r.dy, r.by - (yy - CBCT_MAGIC));
+    const float fz = fmaf(kf, r.dz, r.bz - (yz - CBCT_MAGIC));
+    const unsigned ux = __float_as_uint(yx), uy = __float_as_uint(yy), uz = __float_as_uint(yz);
+    const unsigned t = uy * CBCT_SWIZZLE_Y + uz * CBCT_SWIZZLE_Z;  // magic bits are multiples of 8
+    const unsigned base = (uz * py + uy) * pitch + ux - kfold;
+    const float4 *p00 = packed + (base + (t & 7u));
+    const float4 *p10 = packed + (base + pitch + ((t + CBCT_SWIZZLE_Y) & 7u));
+    const float4 *p01 = packed + (base + plane + ((t + CBCT_SWIZZLE_Z) & 7u));
+    const float4 *p11 = packed + (base + plane + pitch + ((t + CBCT_SWIZZLE_Y + CBCT_SWIZZLE_Z) & 7u));
+    const float4 c000 = __ldg(p00), c100 = __ldg(p00 + 1), c010 = __ldg(p10), c110 = __ldg(p10 + 1);
+    const float4 c001 = __ldg(p01), c101 = __ldg(p01 + 1), c011 = __ldg(p11), c111 = __ldg(p11 + 1);
+    const float gx = 1.0f - fx, gy = 1.0f - fy, gz = 1.0f - fz;
+    const float w00 = gy * gz, w10 = fy * gz, w01 = gy * fz, w11 = fy * fz;
+    const float w000 = gx * w00, w100 = fx * w00, w010 = gx * w10, w110 = fx * w10;
+    const float w001 = gx * w01, w101 = fx * w01, w011 = gx * w11, w111 = fx * w11;
+#define CBCT_TRI(comp) \
+    (fmaf(w000, c000.comp, fmaf(w100, c100.comp, fmaf(w010, c010.comp, w110 * c110.comp))) + \
+     fmaf(w001, c001.comp, fmaf(w101, c101.comp, fmaf(w011, c011.comp, w111 * c111.comp))))
+    A.a0 += CBCT_TRI(x);
+    A.a1 += CBCT_TRI(y);
+    A.a2 += CBCT_TRI(z);
+    A.a3 += CBCT_TRI(w);
+#undef CBCT_TRI
+}
+
+template <int TU>
+__global__ void __launch_bounds__(FP_CTA_U *FP_CTA_V)
+fp4_kernel(const float4 *__restrict__ packed, float *__restrict__ sino, const __grid_constant__ RayGeom G,
+           const __grid_constant__ ViewChunk V, int view0, int accumulate, size_t sino_cstride, int band0,
+           const float *__restrict__ sub)
+{
+    constexpr int TV = 32 / TU, WU = FP_CTA_U / TU;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int iu = blockIdx.x * FP_CTA_U + (warp % WU) * TU + (lane % TU);
+    const int iv = (band0 + blockIdx.z) * FP_CTA_V + (warp / WU) * TV + (lane / TU);
+    if (iu >= G.nu || iv >= G.nv) return;
+    const int view = blockIdx.y;
+    const Ray r = cbct_ray_setup(G, V.cs[view].x, V.cs[view].y, iu, iv);
+    const unsigned py = G.py, pitch = G.px + CBCT_ROW_SKEW, plane = pitch * py;
+    const unsigned kfold = CBCT_MAGIC_BITS * ((py + 1u) * pitch + 1u);  // magic bits of jz, jy, jx through the cell formula
+    Acc4 A = {0.f, 0.f, 0.f, 0.f}, B = {0.f, 0.f, 0.f, 0.f};
+    float kf = r.kf0;
+    int it = 0;
+    for (; it + 1 < r.n; it += 2, kf += 2.0f) {  // even / odd samples into separate sums, as in fp_kernel
+        fp4_sample(packed, r, kf, py, pitch, plane, kfold, A);
+        fp4_sample(packed, r, kf + 1.0f, py, pitch, plane, kfold, B);
+    }
+    if (it < r.n) fp4_sample(packed, r, kf, py, pitch, plane, kfold, A);
+    const float delta = (float)G.delta;
+    const size_t o = ((size_t)(view0 + view) * G.nv + iv) * G.nu + iu;
+    const float acc[4] = {A.a0 + B.a0, A.a1 + B.a1, A.a2 + B.a2, A.a3 + B.a3};
+#pragma unroll
+    for (int c = 0; c < 4; ++c) {
+        float val = acc[c] * delta;
+        if (sub) val -= __ldg(sub + c * sino_cstride + o);
+        float *dst = sino + c * sino_cstride + o;
+        *dst = accumulate ? *dst + val : val;
+    }
+}
+
 __global__ void __launch_bounds__(256) negate_kernel(float *buf, size_t n)
 {
     for (size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x; e < n; e += (size_t)gridDim.x * blockDim.x)
@@ -166,14 +277,30 @@ __global__ void __launch_bounds__(256) negate_kernel(float *buf, size_t n)
 // ---------------------------------------------------------------------------
 size_t cbct_packed_volume_cells(const RayGeom &r) { return (size_t)r.px * r.py * r.pz; }
 
+// Layout of a packed slab of `channels` channels: channels / 4 channel-interleaved groups first, then the
+// remaining channels quad-packed one by one.  Never more than channels * cbct_packed_volume_cells(r) cells.
+static size_t packed_tail_offset(const RayGeom &r, int channels) { return (size_t)(channels / 4) * cbct_packed4_cells(r); }
+
 int cbct_launch_pack_volume(cbct_geom *g, const RayGeom &r, const float *src, float4 *dst, int channels,
                             size_t src_channel_stride, int src_z_origin, cudaStream_t st)
 {
-    int rows = r.py * r.pz;
-    dim3 block(256), grid((r.px + 255) / 256, rows < 148 * 8 ? rows : 148 * 8, channels);
-    pack_volume_kernel<<<grid, block, 0, st>>>(src, dst, r, src_channel_stride, src_z_origin,
-                                               cbct_packed_volume_cells(r));
-    return cbct_check_launch(g, "pack_volume_kernel");
+    const int rows = r.py * r.pz, groups = channels / 4, tail = channels - 4 * groups;
+    const unsigned gy = rows < 148 * 8 ? rows : 148 * 8;
+    if (groups) {
+        dim3 grid((r.px + CBCT_ROW_SKEW + 255) / 256, gy, groups);
+        pack_volume4_kernel<<<grid, 256, 0, st>>>(src, dst, r, src_channel_stride, src_z_origin, 4 * src_channel_stride,
+                                                  cbct_packed4_cells(r));
+        int rc = cbct_check_launch(g, "pack_volume4_kernel");
+        if (rc) return rc;
+    }
+    if (tail) {
+        dim3 grid((r.px + 255) / 256, gy, tail);
+        pack_volume_kernel<<<grid, 256, 0, st>>>(src + (size_t)4 * groups * src_channel_stride,
+                                                 dst + packed_tail_offset(r, channels), r, src_channel_stride,
+                                                 src_z_origin, cbct_packed_volume_cells(r));
+        return cbct_check_launch(g, "pack_volume_kernel");
+    }
+    return CBCT_OK;
 }
 
 template <int CB>
@@ -193,6 +320,21 @@ static int launch_fp_cb(cbct_geom *g, const RayGeom &r, const ViewChunk &vc, int
                                                                band0, sub);
     cbct_prof_end(g, CBCT_KERNEL_FP, st);
     return cbct_check_launch(g, "fp_kernel");
+}
+
+static int launch_fp4(cbct_geom *g, const RayGeom &r, const ViewChunk &vc, int nviews, int view0, const float4 *packed,
+                      float *sino, int accumulate, size_t sstride, int band0, int nbands, const float *sub,
+                      cudaStream_t st)
+{
+    dim3 grid((r.nu + FP_CTA_U - 1) / FP_CTA_U, nviews, nbands);
+    cbct_prof_begin(g, CBCT_KERNEL_FP, st);
+    // warp shape as in launch_fp_cb
+    if (r.z1 - r.z0 >= 64 || r.z1 - r.z0 == r.nz)
+        fp4_kernel<4><<<grid, FP_CTA_U * FP_CTA_V, 0, st>>>(packed, sino, r, vc, view0, accumulate, sstride, band0, sub);
+    else
+        fp4_kernel<8><<<grid, FP_CTA_U * FP_CTA_V, 0, st>>>(packed, sino, r, vc, view0, accumulate, sstride, band0, sub);
+    cbct_prof_end(g, CBCT_KERNEL_FP, st);
+    return cbct_check_launch(g, "fp4_kernel");
 }
 
 int cbct_launch_fp(cbct_geom *g, const RayGeom &r, const float4 *packed, float *sino, int channels, int accumulate,
@@ -223,9 +365,15 @@ int cbct_launch_fp(cbct_geom *g, const RayGeom &r, const float4 *packed, float *
         if (n > CBCT_VIEWS_PER_LAUNCH) n = CBCT_VIEWS_PER_LAUNCH;
         for (int i = 0; i < n; ++i) vc.cs[i] = make_double2(g->cosphi[view0 + i], g->sinphi[view0 + i]);
         int c = 0;
+        for (; c + 4 <= channels; c += 4) {  // channel-interleaved groups
+            int rc = launch_fp4(g, r, vc, n, view0, packed + (size_t)(c / 4) * cbct_packed4_cells(r), sino + c * sstride,
+                                accumulate, sstride, band0, nbands, sub ? sub + c * sstride : nullptr, st);
+            if (rc) return rc;
+        }
+        const float4 *tail = packed + packed_tail_offset(r, channels) - (size_t)c * pstride;
         while (c < channels) {
             int left = channels - c, rc;
-            const float4 *p = packed + c * pstride;
+            const float4 *p = tail + c * pstride;
             float *s = sino + c * sstride;
             // 2 channels per thread measured best at 256^3 (4 lowers occupancy and L1 hit rate)
             if (left >= 2) { rc = launch_fp_cb<2>(g, r, vc, n, view0, p, s, accumulate, pstride, sstride, band0, nbands, sub ? sub + c * sstride : nullptr, st); c += 2; }

@@ -317,9 +317,13 @@ def test_config4_multichannel_sampled(cbct, oracle_mod):
     for c in (0, 1, 7):
         _sampled_checks(oracle_mod, og, vol[c], sino[c], Ax[c], Aty[c], F[c], (41 + c, 51 + c, 61 + c),
                         n_rays=800, n_adj=64, n_fdk=800)
-    # channel independence at full size: channel 3 alone gives the same bits as channel 3 of the batch
+    # channel independence at full size: the batch in reversed channel order (every channel in another group of 4
+    # and another component of its cells) gives the same bits; one channel alone takes the quad-packed kernel,
+    # whose interpolation rounds differently: equal to 1e-6 of the sinogram's scale
+    rev = run_fp(cbct, kw, vol[::-1])
+    assert np.array_equal(rev[::-1], Ax)
     one = run_fp(cbct, kw, vol[3:4])
-    assert np.array_equal(one[0], Ax[3])
+    assert np.max(np.abs(one[0] - Ax[3])) <= 1e-6 * np.max(np.abs(Ax[3]))
 
 
 def test_config5_large_streamed_sampled(cbct, oracle_mod):
@@ -584,16 +588,17 @@ def test_other_ray_steps(cbct, oracle_mod, step):
 
 @pytest.mark.parametrize("pinned", [True, False])
 def test_host_buffers_channel_pipeline(cbct, oracle_mod, pinned):
-    """HOST buffers, 5 channels: the calls run as a 3-stage pipeline over blocks of 2 channels (H2D copy,
-    device implementation, D2H copy; two buffers per side), so 3 blocks exercise the buffer hand-over.
+    """HOST buffers, 9 channels: the calls run as a 3-stage pipeline over blocks of 2 channels (4 for the forward
+    projector: H2D copy, device implementation, D2H copy; two buffers per side), so 3 or more blocks exercise the
+    buffer hand-over.
     Results must equal the oracle and, bit for bit, the same calls on device buffers."""
     kw = dict(synth.geom_kwargs(synth.CONFIGS["tiny"]))
     kw.update(n_views=12, det_off_u_mm=15.0)
     g = cbct.Geometry(**kw)
     og = oracle_mod.Geom(**kw)
     rng = np.random.default_rng(51)
-    vol = rng.random((5,) + g.vol_shape, dtype=np.float32)
-    sino = rng.random((5,) + g.sino_shape, dtype=np.float32)
+    vol = rng.random((9,) + g.vol_shape, dtype=np.float32)
+    sino = rng.random((9,) + g.sino_shape, dtype=np.float32)
 
     def host(a):
         t = torch.from_numpy(a.copy())
@@ -602,16 +607,46 @@ def test_host_buffers_channel_pipeline(cbct, oracle_mod, pinned):
             ("fp", g.fp, vol, g.sino_shape, oracle_mod.fp(og, vol.astype(np.float64)), 1e-5),
             ("adjoint", g.bp_adjoint, sino, g.vol_shape, oracle_mod.bp_adjoint(og, sino.astype(np.float64)), 1e-4),
             ("fdk", g.bp_fdk, sino, g.vol_shape, oracle_mod.bp_fdk(og, sino.astype(np.float64)), 1e-5)):
-        out_h = host(np.full((5,) + shape, np.nan, dtype=np.float32))
-        fn(host(src), out_h, 5)
+        out_h = host(np.full((9,) + shape, np.nan, dtype=np.float32))
+        fn(host(src), out_h, 9)
         torch.cuda.synchronize()
-        out_d = torch.empty((5,) + shape, device="cuda")
-        fn(dev(src), out_d, 5)
+        out_d = torch.empty((9,) + shape, device="cuda")
+        fn(dev(src), out_d, 9)
         torch.cuda.synchronize()
         assert rel_l2(out_h.numpy().astype(np.float64), ref) <= tol, name
         assert np.array_equal(out_h.numpy(), out_d.cpu().numpy()), name
         # mixed: host input, device output
-        out_m = torch.empty((5,) + shape, device="cuda")
-        fn(host(src), out_m, 5)
+        out_m = torch.empty((9,) + shape, device="cuda")
+        fn(host(src), out_m, 9)
         torch.cuda.synchronize()
         assert torch.equal(out_m, out_d), name
+
+
+@pytest.mark.parametrize("C,cap,over", [(4, 0, dict()), (7, 0, dict(vol_nx=37, vol_ny=29, vol_nz=21, vol_cx_mm=5.0, det_off_v_mm=-4.0)),
+                                        (9, 0, dict(n_views=7)), (6, 6000000, dict(vol_nz=40, n_views=12, det_off_u_mm=15.0))])
+def test_fp_channel_groups(cbct, oracle_mod, C, cap, over):
+    """Forward projector with 4 or more channels: groups of 4 go through the channel-interleaved layout
+    (fp4_kernel), the remainder through the quad-packed one; resident and z-slab paths, with and without the
+    fused residual, against the oracle channel by channel."""
+    kw = dict(synth.geom_kwargs(synth.CONFIGS["tiny"]))
+    kw.update(over)
+    g = cbct.Geometry(**kw, max_workset_bytes=cap)
+    if cap:
+        assert g.num_slabs(C) > 2
+    og = oracle_mod.Geom(**kw)
+    rng = np.random.default_rng(61 + C)
+    vol = rng.random((C,) + g.vol_shape, dtype=np.float32)
+    vol[1] -= 0.5   # one signed channel
+    y = rng.random((C,) + g.sino_shape, dtype=np.float32) * 50.0
+    ref = oracle_mod.fp(og, vol.astype(np.float64))
+    out = torch.full((C,) + g.sino_shape, float("nan"), device="cuda")
+    g.fp(dev(vol), out, C)
+    got = out.cpu().numpy().astype(np.float64)
+    for c in range(C):
+        if c != 1:
+            assert rel_l2(got[c], ref[c]) <= 1e-5 and max_rel(got[c], ref[c]) <= 1e-4, c
+    scale = float(np.max(np.abs(ref[0])))
+    assert np.max(np.abs(got[1] - ref[1])) <= 1e-5 * scale
+    g.fp_residual(dev(vol), dev(y), out, C)
+    got = out.cpu().numpy().astype(np.float64)
+    assert np.max(np.abs(got - (ref - y))) <= 2e-5 * scale
