@@ -30,7 +30,7 @@ UNIT = "Gsamples/s"
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of each kernel at the default workload,
 # from the ncu --set full capture summarised in profiles/r1_final.md (multichannel_256; fp and adjoint launches
 # carry 2 channels, fdk launches 1).  Reported only for that workload.
-NCU_DRAM_BYTES_PER_LAUNCH = {"fp_kernel": 0.732e9, "adjoint_gather_kernel": 1.946e9, "fdk_kernel": 0.206e9}
+NCU_DRAM_BYTES_PER_LAUNCH = {"fp4_pair_kernel": 0.581e9, "adjoint_gather_kernel": 1.946e9, "fdk_kernel": 0.206e9}
 
 
 def peaks():
@@ -198,7 +198,9 @@ def main():
         cdist.barrier(cuda=True)
     g.profile(False)
     launches = g.launch_count() - l0
-    kern = {name: g.profile_read(i) for i, name in enumerate(("fp_kernel", "adjoint_gather_kernel", "fdk_kernel"))}
+    # groups of 4 channels go through fp4_pair_kernel, the remaining channels through fp_kernel (one timing slot)
+    fp_name = "fp_kernel" if C < 4 else ("fp4_pair_kernel" if C % 4 == 0 else "fp4_pair_kernel+fp_kernel")
+    kern = {name: g.profile_read(i) for i, name in enumerate((fp_name, "adjoint_gather_kernel", "fdk_kernel"))}
     t_fp = sum(e[0].elapsed_time(e[1]) for e in evs) / args.steps
     t_adj = sum(e[1].elapsed_time(e[2]) for e in evs) / args.steps
     t_fdk = sum(e[2].elapsed_time(e[3]) for e in evs) / args.steps
@@ -300,7 +302,7 @@ def main():
     # 148 SMs x 128 B/clk x the SM clock sampled during the timed region.  Launch durations are the
     # library's own CUDA-event pairs around each kernel launch, on the launching stream.
     l1_peak = 148 * 128 * sm_hz / 1e9
-    work = {"fp_kernel": 32.0 * C * n_samples, "adjoint_gather_kernel": 64.0 * C * n_samples,
+    work = {fp_name: 32.0 * C * n_samples, "adjoint_gather_kernel": 64.0 * C * n_samples,
             "fdk_kernel": 16.0 * C * n_vv}     # algorithmic bytes per step
     per_kernel = {}
     for name, (ms, n) in kern.items():

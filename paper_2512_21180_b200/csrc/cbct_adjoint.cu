@@ -80,10 +80,10 @@ interleave_views_kernel(const float *__restrict__ in, float *__restrict__ out, i
 // (iu, iv) ranges (measured 32.0 -> 29.5 ms per channel against 32 x 1; 4 x 8 and 8 x 2 x 2: 29.8, 29.7).
 #define ADJ_BX 8
 #define ADJ_BY 16
-#define ADJ_BZ 1
 
-template <int NR, int NM, int CB, bool FINE>
-__global__ void __launch_bounds__(ADJ_BX *ADJ_BY *ADJ_BZ)
+// ADJ_BZ planes per CTA; MINB = CTAs per SM the register allocation aims for (0: the compiler's choice)
+template <int NR, int NM, int CB, bool FINE, int ADJ_BZ, int MINB>
+__global__ void __launch_bounds__(ADJ_BX *ADJ_BY *ADJ_BZ, MINB)
 adjoint_gather_kernel(const float *__restrict__ sinoI, float *__restrict__ vol, const __grid_constant__ AdjGeom G,
                       const __grid_constant__ ViewChunk V, int q0, int accumulate, size_t sino_cstride,
                       size_t vol_cstride, int vol_z_origin)
@@ -93,23 +93,37 @@ adjoint_gather_kernel(const float *__restrict__ sinoI, float *__restrict__ vol, 
     const int nzb = (G.bz1 - G.bz0 + ADJ_BZ - 1) / ADJ_BZ;
     const int split = blockIdx.z / nzb;
     const int iz = G.bz0 + (blockIdx.z - split * nzb) * ADJ_BZ + threadIdx.z;
-    if (ix >= G.bx || iy >= G.by || iz >= G.bz1) return;
+    const bool valid = ix < G.bx && iy < G.by && iz < G.bz1;
     vol += split * G.split_stride;
     const int q_begin = split * G.views_per_split, q_end = min(G.nq, q_begin + G.views_per_split);
     const double X = G.x0 + ix, Y = G.y0 + iy, Z = G.z0 + iz;
-    float acc[NM][CB][NR];
+    // Sums over views: registers up to 16 per thread, beyond that a private column of shared memory (touched
+    // once per view, so its traffic is nothing; it keeps 4 channels x 8 symmetric voxels at the register count
+    // of 2 channels).
+    constexpr int NACC = NM * CB * NR;
+    constexpr bool SACC = NACC > 16;
+    constexpr int NT = ADJ_BX * ADJ_BY * ADJ_BZ;
+    __shared__ float sacc[SACC ? NACC : 1][SACC ? NT : 1];
+    const int tid = threadIdx.x + ADJ_BX * (threadIdx.y + ADJ_BY * threadIdx.z);
+    float acc[SACC ? 1 : NM][SACC ? 1 : CB][SACC ? 1 : NR];
+    if (SACC) {
 #pragma unroll
-    for (int m = 0; m < NM; ++m)
+        for (int i = 0; i < NACC; ++i) sacc[SACC ? i : 0][SACC ? tid : 0] = 0.f;
+    } else {
 #pragma unroll
-        for (int c = 0; c < CB; ++c)
+        for (int m = 0; m < NM; ++m)
 #pragma unroll
-            for (int r = 0; r < NR; ++r) acc[m][c][r] = 0.f;
+            for (int c = 0; c < CB; ++c)
+#pragma unroll
+                for (int r = 0; r < NR; ++r) acc[SACC ? 0 : m][SACC ? 0 : c][SACC ? 0 : r] = 0.f;
+    }
     const float u0f = (float)G.u0, duf = (float)G.du, v0f = (float)G.v0, dvf = (float)G.dv;
     const float sddf = (float)G.sdd, sdd2f = (float)(G.sdd * G.sdd), inv_stepf = (float)G.inv_step;
     const float zcull = 1.4143f * (float)G.inv_sdd;
     const size_t img = (size_t)G.nv * G.nu;
 
     for (int q = q_begin; q < q_end; ++q) {
+        if (!valid) continue;
         // ---- fp64 set-up of the voxel's projection (once per voxel and view) ----
         const double c = V.cs[q].x, s = V.cs[q].y;
         const double U = G.sid - (X * c + Y * s), w = Y * c - X * s;
@@ -213,10 +227,14 @@ adjoint_gather_kernel(const float *__restrict__ sinoI, float *__restrict__ vol, 
             for (int cc = 0; cc < CB; ++cc) {
                 rotate_views<NR>(accv[m][cc], a);
 #pragma unroll
-                for (int r = 0; r < NR; ++r) acc[m][cc][r] += accv[m][cc][r];
+                for (int r = 0; r < NR; ++r) {
+                    if (SACC) sacc[SACC ? (m * CB + cc) * NR + r : 0][SACC ? tid : 0] += accv[m][cc][r];
+                    else acc[SACC ? 0 : m][SACC ? 0 : cc][SACC ? 0 : r] += accv[m][cc][r];
+                }
             }
     }
 
+    if (!valid) return;
     // ---- stores: rotation r maps (ix, iy) -> r quarter (NR = 4) or half (NR = 2) turns ----
 #pragma unroll
     for (int m = 0; m < NM; ++m) {
@@ -235,7 +253,8 @@ adjoint_gather_kernel(const float *__restrict__ sinoI, float *__restrict__ vol, 
             const size_t o = ((size_t)(z - vol_z_origin) * G.ny + y) * G.nx + x;
 #pragma unroll
             for (int cc = 0; cc < CB; ++cc) {
-                float val = acc[m][cc][r] * G.scale;
+                float val = (SACC ? sacc[SACC ? (m * CB + cc) * NR + r : 0][SACC ? tid : 0]
+                                  : acc[SACC ? 0 : m][SACC ? 0 : cc][SACC ? 0 : r]) * G.scale;
                 float *dst = vol + cc * vol_cstride + o;
                 *dst = accumulate ? *dst + val : val;
             }
@@ -274,7 +293,7 @@ reduce_splits_kernel(const float *__restrict__ partial, float *__restrict__ out,
     }
 }
 
-template <int NR, int NM, int CB>
+template <int NR, int NM, int CB, int ADJ_BZ = 1, int MINB = 0>
 static int launch_gather(cbct_geom *g, AdjGeom &G, const float *sinoI, float *vol, int accumulate_first,
                          size_t sstride, size_t vstride, int vol_z_origin, float *partial, int nsplit, cudaStream_t st)
 {
@@ -295,8 +314,8 @@ static int launch_gather(cbct_geom *g, AdjGeom &G, const float *sinoI, float *vo
         G.split_stride = (size_t)CB * nvox;
         grid.z = nzb * nsplit;
         cbct_prof_begin(g, CBCT_KERNEL_ADJOINT, st);
-        if (G.step < 0.5f) adjoint_gather_kernel<NR, NM, CB, true><<<grid, block, 0, st>>>(sinoI, partial, G, vc, 0, 0, sstride, nvox, 0);
-        else adjoint_gather_kernel<NR, NM, CB, false><<<grid, block, 0, st>>>(sinoI, partial, G, vc, 0, 0, sstride, nvox, 0);
+        if (G.step < 0.5f) adjoint_gather_kernel<NR, NM, CB, true, ADJ_BZ, MINB><<<grid, block, 0, st>>>(sinoI, partial, G, vc, 0, 0, sstride, nvox, 0);
+        else adjoint_gather_kernel<NR, NM, CB, false, ADJ_BZ, MINB><<<grid, block, 0, st>>>(sinoI, partial, G, vc, 0, 0, sstride, nvox, 0);
         cbct_prof_end(g, CBCT_KERNEL_ADJOINT, st);
         int rc = cbct_check_launch(g, "adjoint_gather_kernel");
         if (rc) return rc;
@@ -312,10 +331,10 @@ static int launch_gather(cbct_geom *g, AdjGeom &G, const float *sinoI, float *vo
         G.nq = n;
         cbct_prof_begin(g, CBCT_KERNEL_ADJOINT, st);
         if (G.step < 0.5f)
-            adjoint_gather_kernel<NR, NM, CB, true><<<grid, block, 0, st>>>(sinoI, vol, G, vc, q0, accumulate_first || q0 > 0,
+            adjoint_gather_kernel<NR, NM, CB, true, ADJ_BZ, MINB><<<grid, block, 0, st>>>(sinoI, vol, G, vc, q0, accumulate_first || q0 > 0,
                                                                             sstride, vstride, vol_z_origin);
         else
-            adjoint_gather_kernel<NR, NM, CB, false><<<grid, block, 0, st>>>(sinoI, vol, G, vc, q0, accumulate_first || q0 > 0,
+            adjoint_gather_kernel<NR, NM, CB, false, ADJ_BZ, MINB><<<grid, block, 0, st>>>(sinoI, vol, G, vc, q0, accumulate_first || q0 > 0,
                                                                              sstride, vstride, vol_z_origin);
         cbct_prof_end(g, CBCT_KERNEL_ADJOINT, st);
         int rc = cbct_check_launch(g, "adjoint_gather_kernel");
@@ -334,9 +353,18 @@ static int launch_gather_channels(cbct_geom *g, AdjGeom &G, const float *sinoI, 
         int left = channels - c, rc;
         const float *s = sinoI + c * sstride;
         float *v = vol + c * vstride;
-        // One weight evaluation feeds NR * NM * CB accumulators; 16 is the sweet spot (with all symmetries, 2
-        // channels: 4 need 128 registers and measured slower, 158 vs 143 ms at C = 8).  Geometries with fewer
+        // One weight evaluation feeds NR * NM * CB accumulators: 16 in registers; geometries with fewer
         // symmetries (irregular view angles, off-centre grids) make it up with more channels per thread.
+        // 32 accumulators per weight evaluation when the channels are there; the sums over views then live in
+        // shared memory and the CTA is 8 x 16 x 2 voxels, 2 CTAs = 16 warps per SM (measured at 256^3 / 400 views,
+        // 8 channels: 17.5 -> 12.8 ms per channel; with 128-thread CTAs the 20 resident warps drift apart by
+        // several views and evict each other's pixels from L1: hit rate 56 %, no gain)
+        if constexpr (NR * NM == 8) {
+            if (left >= 4) { rc = launch_gather<NR, NM, 4, 2, 2>(g, G, s, v, 0, sstride, vstride, vol_z_origin, partial, nsplit, st); c += 4; if (rc) return rc; continue; }
+        }
+        if constexpr (NR * NM == 4) {
+            if (left >= 8) { rc = launch_gather<NR, NM, 8, 2, 2>(g, G, s, v, 0, sstride, vstride, vol_z_origin, partial, nsplit, st); c += 8; if (rc) return rc; continue; }
+        }
         if constexpr (NR * NM <= 2) {
             if (left >= 8) { rc = launch_gather<NR, NM, 8>(g, G, s, v, 0, sstride, vstride, vol_z_origin, partial, nsplit, st); c += 8; if (rc) return rc; continue; }
         }

@@ -231,39 +231,44 @@ __device__ __forceinline__ void fp4_sample(const float4 *__restrict__ packed, co
 #undef CBCT_TRI
 }
 
-template <int TU>
-__global__ void __launch_bounds__(FP_CTA_U *FP_CTA_V)
-fp4_kernel(const float4 *__restrict__ packed, float *__restrict__ sino, const __grid_constant__ RayGeom G,
-           const __grid_constant__ ViewChunk V, int view0, int accumulate, size_t sino_cstride, int band0,
-           const float *__restrict__ sub)
+// Two lanes per ray: lane 2m takes the even samples of ray m, lane 2m + 1 the odd ones (the same two sums as
+// fp_kernel's acc / acc2), so a quarter-warp -- the unit the L1 data stage serves per cycle -- covers 2 x 2 pixels
+// x 2 consecutive samples instead of 4 x 2 pixels: fewer distinct cells and lines per quarter-warp (measured 4.9
+// data-stage cycles per LDG.128 against 5.9 with one lane per ray; the floor is 4.1).  A warp covers 4 x 4
+// pixels, a CTA 16 x 8.  (The same split does not pay for fp_kernel, whose extra cycles are fills.)
+__global__ void __launch_bounds__(256)
+fp4_pair_kernel(const float4 *__restrict__ packed, float *__restrict__ sino, const __grid_constant__ RayGeom G,
+                const __grid_constant__ ViewChunk V, int view0, int accumulate, size_t sino_cstride, int band0,
+                const float *__restrict__ sub)
 {
-    constexpr int TV = 32 / TU, WU = FP_CTA_U / TU;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int iu = blockIdx.x * FP_CTA_U + (warp % WU) * TU + (lane % TU);
-    const int iv = (band0 + blockIdx.z) * FP_CTA_V + (warp / WU) * TV + (lane / TU);
-    if (iu >= G.nu || iv >= G.nv) return;
+    const int par = lane & 1;
+    const int iu = blockIdx.x * 16 + (warp & 3) * 4 + ((lane >> 1) & 1) + ((lane >> 3) & 1) * 2;
+    const int iv = (band0 + blockIdx.z) * 8 + (warp >> 2) * 4 + ((lane >> 2) & 1) + ((lane >> 4) & 1) * 2;
+    const bool inside = iu < G.nu && iv < G.nv;
     const int view = blockIdx.y;
-    const Ray r = cbct_ray_setup(G, V.cs[view].x, V.cs[view].y, iu, iv);
+    Ray r = cbct_ray_setup(G, V.cs[view].x, V.cs[view].y, inside ? iu : 0, inside ? iv : 0);
+    if (!inside) r.n = 0;
     const unsigned py = G.py, pitch = G.px + CBCT_ROW_SKEW, plane = pitch * py;
-    const unsigned kfold = CBCT_MAGIC_BITS * ((py + 1u) * pitch + 1u);  // magic bits of jz, jy, jx through the cell formula
-    Acc4 A = {0.f, 0.f, 0.f, 0.f}, B = {0.f, 0.f, 0.f, 0.f};
-    float kf = r.kf0;
-    int it = 0;
-    for (; it + 1 < r.n; it += 2, kf += 2.0f) {  // even / odd samples into separate sums, as in fp_kernel
-        fp4_sample(packed, r, kf, py, pitch, plane, kfold, A);
-        fp4_sample(packed, r, kf + 1.0f, py, pitch, plane, kfold, B);
-    }
-    if (it < r.n) fp4_sample(packed, r, kf, py, pitch, plane, kfold, A);
+    const unsigned kfold = CBCT_MAGIC_BITS * ((py + 1u) * pitch + 1u);
+    Acc4 A = {0.f, 0.f, 0.f, 0.f};
+    float kf = r.kf0 + (float)par;
+    for (int it = par; it < r.n; it += 2, kf += 2.0f) fp4_sample(packed, r, kf, py, pitch, plane, kfold, A);
+    A.a0 += __shfl_xor_sync(0xffffffffu, A.a0, 1);
+    A.a1 += __shfl_xor_sync(0xffffffffu, A.a1, 1);
+    A.a2 += __shfl_xor_sync(0xffffffffu, A.a2, 1);
+    A.a3 += __shfl_xor_sync(0xffffffffu, A.a3, 1);
+    if (!inside) return;
     const float delta = (float)G.delta;
     const size_t o = ((size_t)(view0 + view) * G.nv + iv) * G.nu + iu;
-    const float acc[4] = {A.a0 + B.a0, A.a1 + B.a1, A.a2 + B.a2, A.a3 + B.a3};
-#pragma unroll
-    for (int c = 0; c < 4; ++c) {
-        float val = acc[c] * delta;
-        if (sub) val -= __ldg(sub + c * sino_cstride + o);
-        float *dst = sino + c * sino_cstride + o;
-        *dst = accumulate ? *dst + val : val;
-    }
+    // lane 2m stores channels 0 and 1, lane 2m + 1 channels 2 and 3
+    const float lo = par ? A.a2 : A.a0, hi = par ? A.a3 : A.a1;
+    const int c0 = 2 * par;
+    float val = lo * delta, val2 = hi * delta;
+    if (sub) { val -= __ldg(sub + c0 * sino_cstride + o); val2 -= __ldg(sub + (c0 + 1) * sino_cstride + o); }
+    float *dst = sino + c0 * sino_cstride + o, *dst2 = dst + sino_cstride;
+    *dst = accumulate ? *dst + val : val;
+    *dst2 = accumulate ? *dst2 + val2 : val2;
 }
 
 __global__ void __launch_bounds__(256) negate_kernel(float *buf, size_t n)
@@ -326,15 +331,12 @@ static int launch_fp4(cbct_geom *g, const RayGeom &r, const ViewChunk &vc, int n
                       float *sino, int accumulate, size_t sstride, int band0, int nbands, const float *sub,
                       cudaStream_t st)
 {
-    dim3 grid((r.nu + FP_CTA_U - 1) / FP_CTA_U, nviews, nbands);
     cbct_prof_begin(g, CBCT_KERNEL_FP, st);
-    // warp shape as in launch_fp_cb
-    if (r.z1 - r.z0 >= 64 || r.z1 - r.z0 == r.nz)
-        fp4_kernel<4><<<grid, FP_CTA_U * FP_CTA_V, 0, st>>>(packed, sino, r, vc, view0, accumulate, sstride, band0, sub);
-    else
-        fp4_kernel<8><<<grid, FP_CTA_U * FP_CTA_V, 0, st>>>(packed, sino, r, vc, view0, accumulate, sstride, band0, sub);
+    // 16 x 8-pixel CTAs: twice as many bands of half the height as the caller counted
+    dim3 grid2((r.nu + 15) / 16, nviews, 2 * nbands);
+    fp4_pair_kernel<<<grid2, 256, 0, st>>>(packed, sino, r, vc, view0, accumulate, sstride, 2 * band0, sub);
     cbct_prof_end(g, CBCT_KERNEL_FP, st);
-    return cbct_check_launch(g, "fp4_kernel");
+    return cbct_check_launch(g, "fp4_pair_kernel");
 }
 
 int cbct_launch_fp(cbct_geom *g, const RayGeom &r, const float4 *packed, float *sino, int channels, int accumulate,
