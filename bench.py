@@ -28,9 +28,9 @@ UNIT = "Gsamples/s"
 
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of each kernel at the default workload,
-# from the ncu --set full capture summarised in profiles/r1_final.md (multichannel_256; fp and adjoint launches
-# carry 2 channels, fdk launches 1).  Reported only for that workload.
-NCU_DRAM_BYTES_PER_LAUNCH = {"fp4_pair_kernel": 0.581e9, "adjoint_gather_kernel": 1.946e9, "fdk_kernel": 0.206e9}
+# from the ncu --set full captures summarised in profiles/r1_final.md (multichannel_256; fp and adjoint launches
+# carry 4 channels, fdk launches 1).  Reported only for that workload.
+NCU_DRAM_BYTES_PER_LAUNCH = {"fp4_pair_kernel": 0.583e9, "adjoint_gather_kernel": 0.278e9, "fdk_kernel": 0.209e9}
 
 
 def peaks():
@@ -248,6 +248,17 @@ def main():
                       "downsample2_ms": t_dn, "downsample2_hbm_gbs": (vol_h.nbytes * 1.125) / (t_dn * 1e-3) / 1e9,
                       "upsample2_ms": t_up, "upsample2_hbm_gbs": (vol_h.nbytes * 1.125) / (t_up * 1e-3) / 1e9,
                       "proj_down2_ms": t_pd, "proj_down2_hbm_gbs": (sino_h.nbytes * 0.5 * 1.25) / (t_pd * 1e-3) / 1e9})
+
+        if C >= 2:
+            # NEXT-4: water-bone decomposition of one volume; noise-free polychromatic signal of one sinogram pair
+            _, mu_w, mu_b, i0 = synth.spectrum_tables(cfg["det_nv"], cfg["det_nu"])
+            d_i0 = torch.from_numpy(i0).cuda()
+            resp = [5.0 + 0.375 * (e - 20.0) if e <= 60.0 else 20.0 - (e - 60.0) / 6.0 for e in (25.0 + 10.0 * np.arange(10))]
+            t_wb = timed(lambda: cbct.water_bone(vol[0], vol_out[0], vol_out[1]))
+            t_poly = timed(lambda: cbct.polychromatic_primary(sino_in[0], sino_in[1], d_i0, mu_w, mu_b, resp, sino_out[0]))
+            next1.update({"water_bone_ms": t_wb, "water_bone_hbm_gbs": 3 * vol_h[0].nbytes / (t_wb * 1e-3) / 1e9,
+                          "polychromatic_primary_ms": t_poly,
+                          "polychromatic_primary_hbm_gbs": 3 * sino_h[0].nbytes / (t_poly * 1e-3) / 1e9})
 
     # end to end through the C ABI with HOST (pinned) buffers: copies inside the timed region
     e2e = None
