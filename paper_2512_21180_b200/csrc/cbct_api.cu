@@ -89,7 +89,7 @@ static int begin_call(const cbct_geom *gc, const void *vol, const void *sino, in
 // A2 + A5
 // ---------------------------------------------------------------------------
 // ---------------------------------------------------------------------------
-// HOST buffers without a work-set cap: the call is cut into blocks of 2 channels (4 for the forward projector) that flow through a
+// HOST buffers without a work-set cap: the call is cut into blocks of 2 channels (4 for the forward projector and the adjoint) that flow through a
 // three-stage pipeline -- H2D copy of block b+1 (one stream), the device implementation on block b (the
 // caller's stream), D2H copy of block b-1 (another stream) -- with two device buffers per side, so the
 // PCIe copies in both directions hide behind the kernels.  `inner(din, dout, c0, nc)` enqueues the
@@ -315,7 +315,8 @@ static int adjoint_impl(const cbct_geom *gc, const float *sino, float *vol, int3
         return blocked_call(cx, sino, cx.nsino, cx.ks, vol, cx.nvol, cx.kv,
                             [&](const float *ds, float *dv, int, int nc) {
                                 return adjoint_impl(gc, ds, dv, nc, stream, weighted);
-                            });
+                            },
+                            channels >= 4 ? 4 : 2);  // blocks of 4 channels take the 32-accumulator kernel
 
     const float *d_sino = sino;
     if (cx.ks != MEM_DEVICE) {

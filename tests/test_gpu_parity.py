@@ -589,7 +589,7 @@ def test_other_ray_steps(cbct, oracle_mod, step):
 @pytest.mark.parametrize("pinned", [True, False])
 def test_host_buffers_channel_pipeline(cbct, oracle_mod, pinned):
     """HOST buffers, 9 channels: the calls run as a 3-stage pipeline over blocks of 2 channels (4 for the forward
-    projector: H2D copy, device implementation, D2H copy; two buffers per side), so 3 or more blocks exercise the
+    projector and the adjoint: H2D copy, device implementation, D2H copy; two buffers per side), so 3 or more blocks exercise the
     buffer hand-over.
     Results must equal the oracle and, bit for bit, the same calls on device buffers."""
     kw = dict(synth.geom_kwargs(synth.CONFIGS["tiny"]))
