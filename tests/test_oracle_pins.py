@@ -382,6 +382,18 @@ def test_p17_water_bone_and_polychromatic(oracle_mod):
     0 at tau_1, kappa_b tau_2 at tau_2), water = rho_hat for soft tissue, bone = kappa_b rho_hat above tau_2;
     one energy bin reduces Eq. 6 to Beer-Lambert; bins add."""
     o = oracle_mod
+    gold = {}
+    for line in open(os.path.join(os.path.dirname(__file__), "golden", "paper_polychromatic.txt")):
+        line = line.split("#")[0].split()
+        if len(line) == 2:
+            gold[line[0]] = float(line[1])
+    # the oracle's defaults and the synthetic energy grid are the paper's printed constants
+    import inspect
+    dflt = {k: v.default for k, v in inspect.signature(o.water_bone).parameters.items() if v.default is not inspect.Parameter.empty}
+    assert (dflt["tau1"], dflt["tau2"], dflt["kappa_b"]) == (gold["tau_1"], gold["tau_2"], gold["kappa_b"])
+    assert list(o.detector_response([20, 60, 120])) == [gold["resp_20_kev"], gold["resp_60_kev"], gold["resp_120_kev"]]
+    en = synth.spectrum_tables(4, 4)[0]
+    assert len(en) == gold["n_energy_bins"] and en[0] == gold["first_bin_centre_kev"] and en[-1] == gold["last_bin_centre_kev"]
     assert list(o.detector_response([20, 60, 120])) == [5.0, 20.0, 10.0]
     assert o.detector_response(25.0) == pytest.approx(5.0 + 15.0 * 5.0 / 40.0) and o.detector_response(115.0) == pytest.approx(10.0 + 10.0 * 5.0 / 60.0)
     eps = 1e-12
