@@ -69,7 +69,6 @@ pack_volume_kernel(const float *__restrict__ src, float4 *__restrict__ dst, cons
 // (CBCT_SWIZZLE_Y jy + CBCT_SWIZZLE_Z jz) mod 8 cells into a pitch of px + 8, which gives cell jx the same
 // 16-byte line position (jx + 6 jy + 4 jz) mod 8 as the rotation does and keeps jx + 1 one cell further.
 // ---------------------------------------------------------------------------
-#define CBCT_ROW_SKEW 8
 __host__ __device__ __forceinline__ size_t cbct_packed4_cells(const RayGeom &r)
 {
     return (size_t)(r.px + CBCT_ROW_SKEW) * r.py * r.pz;

@@ -205,7 +205,8 @@ extern "C" int cbct_geom_count_samples(const cbct_geom *gc, uint64_t *out)
 
 // z-slab plan (A5) of the forward projector: planes per slab so that two slab
 // buffers of all `channels` channels fit under max_workset_bytes.  A slab buffer
-// holds the quad-packed cells (16 B per padded cell) plus the raw planes they
+// holds the packed cells (16 B per padded cell: one per voxel and channel when quad-packed, one per voxel and
+// group of 4 channels when channel-interleaved, cbct_fp.cu) plus the raw planes they
 // are packed from when the caller's volume is in host memory (4 B per voxel;
 // counted always, so the plan does not depend on where the volume lives).
 // Returns planes per slab (nz when everything is resident) or <= 0 if not even
@@ -214,7 +215,9 @@ int cbct_plan_slab_planes(const cbct_geom *g, int channels)
 {
     RayGeom r = cbct_make_raygeom(g, 0, g->d.vol_nz);
     uint64_t cap = g->d.max_workset_bytes;
-    uint64_t packed_plane = (uint64_t)r.px * r.py * 16u * (uint64_t)channels;
+    // groups of 4 channels share one channel-interleaved cell per voxel (row pitch px + 8), the rest are quad-packed
+    uint64_t packed_plane = (uint64_t)(channels / 4) * (uint64_t)(r.px + CBCT_ROW_SKEW) * r.py * 16u
+                            + (uint64_t)(channels % 4) * (uint64_t)r.px * r.py * 16u;
     uint64_t raw_plane = (uint64_t)r.nx * r.ny * 4u * (uint64_t)channels;
     if (cap == 0 || packed_plane * (uint64_t)r.pz + raw_plane * (uint64_t)r.nz <= cap) return g->d.vol_nz;
     int64_t planes = ((int64_t)(cap / 2) - (int64_t)(packed_plane * 2 * CBCT_PAD)) / (int64_t)(packed_plane + raw_plane);

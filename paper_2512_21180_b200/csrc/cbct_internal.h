@@ -21,6 +21,7 @@
 // (jx & ~7) | ((jx + CBCT_SWIZZLE_Y jy + CBCT_SWIZZLE_Z jz) & 7) of its row (cbct_fp.cu)
 #define CBCT_SWIZZLE_Y 6
 #define CBCT_SWIZZLE_Z 4
+#define CBCT_ROW_SKEW 8          // extra cells per row of the channel-interleaved (skewed) layout (cbct_fp.cu)
 
 // View-independent geometry in voxel units (fp64), passed by value to kernels.
 struct RayGeom {

@@ -71,12 +71,15 @@ def test_slab_plan(cbct):
     kw = synth.geom_kwargs(synth.CONFIGS["large_512"])
     assert cbct.Geometry(**kw).num_slabs(4) == 1
     g = cbct.Geometry(**kw, max_workset_bytes=1 << 30)
-    # per plane and 4 channels: 520 x 516 quad-packed cells (16 B; rows padded to whole 128-B lines)
-    # + 512 x 512 raw voxels (4 B);
+    # per plane and 4 channels: (520 + 8) x 516 channel-interleaved cells (16 B for the 4 channels of a voxel; rows
+    # padded to whole 128-B lines plus the skew) + 4 x 512 x 512 raw voxels (4 B);
     # two slab buffers, each with 2 * 2 border planes of packed cells, under 1 GiB
-    packed, raw = 4 * 520 * 516 * 16, 4 * 512 * 512 * 4
+    packed, raw = 528 * 516 * 16, 4 * 512 * 512 * 4
     planes = ((1 << 30) // 2 - 4 * packed) // (packed + raw)
-    assert g.num_slabs(4) == -(-512 // planes)
+    assert g.num_slabs(4) == -(-512 // planes) == 9
+    # 3 channels are quad-packed (16 B per voxel and channel)
+    packed3, raw3 = 3 * 520 * 516 * 16, 3 * 512 * 512 * 4
+    assert g.num_slabs(3) == -(-512 // (((1 << 30) // 2 - 4 * packed3) // (packed3 + raw3)))
     assert g.num_slabs(1) > 1  # one channel quad-packed: 520 * 516^2 * 16 B = 2.2 GB does not fit
     assert cbct.Geometry(**kw, max_workset_bytes=3 << 30).num_slabs(1) == 1
     with pytest.raises(cbct.CbctError, match="NOMEM"):

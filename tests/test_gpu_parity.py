@@ -623,7 +623,7 @@ def test_host_buffers_channel_pipeline(cbct, oracle_mod, pinned):
 
 
 @pytest.mark.parametrize("C,cap,over", [(4, 0, dict()), (7, 0, dict(vol_nx=37, vol_ny=29, vol_nz=21, vol_cx_mm=5.0, det_off_v_mm=-4.0)),
-                                        (9, 0, dict(n_views=7)), (6, 6000000, dict(vol_nz=40, n_views=12, det_off_u_mm=15.0))])
+                                        (9, 0, dict(n_views=7)), (6, 2000000, dict(vol_nz=40, n_views=12, det_off_u_mm=15.0))])
 def test_fp_channel_groups(cbct, oracle_mod, C, cap, over):
     """Forward projector with 4 or more channels: groups of 4 go through the channel-interleaved layout
     (fp4_kernel), the remainder through the quad-packed one; resident and z-slab paths, with and without the
