@@ -42,6 +42,7 @@ struct AdjGeom {
     int nu, nv, nx, ny, nz;
     int bx, by;                             // base domain: ix < bx, iy < by
     int bz0, bz1;                           // base planes [bz0, bz1)
+    int mz_origin;                          // first stored plane of the z-mirrored voxels' output (NM = 2)
     int nq;                                 // views in this launch
     int nbase;                              // n_views / NR: views i and i + nbase differ by 360/NR degrees
     // small grids do not fill the GPU with one thread per base voxel: the views of a launch are then split
@@ -250,7 +251,7 @@ adjoint_gather_kernel(const float *__restrict__ sinoI, float *__restrict__ vol, 
             } else if (NR == 2 && r == 1) {
                 x = G.nx - 1 - ix; y = G.ny - 1 - iy;
             }
-            const size_t o = ((size_t)(z - vol_z_origin) * G.ny + y) * G.nx + x;
+            const size_t o = ((size_t)(z - (m == 0 ? vol_z_origin : G.mz_origin)) * G.ny + y) * G.nx + x;
 #pragma unroll
             for (int cc = 0; cc < CB; ++cc) {
                 float val = (SACC ? sacc[SACC ? (m * CB + cc) * NR + r : 0][SACC ? tid : 0]
@@ -401,9 +402,15 @@ int cbct_adjoint_view_splits(const cbct_geom *g)
 
 // `partial` (nsplit > 1 only): workspace of nsplit * 8 * nx * ny * nz floats; used when the launch covers the
 // whole grid (zs0 = 0, zs1 = nz, vol_z_origin = 0).
+// mirror_z_origin != CBCT_NO_MIRROR_PAIR (z-slab streaming of a z-symmetric geometry): planes [zs0, zs1) lie in
+// the lower half of the grid and the launch also fills their mirror images [nz - zs1, nz - zs0), stored from
+// plane index mirror_z_origin of the same buffer.
 int cbct_launch_adjoint(cbct_geom *g, const float *sino_src, float *vol, int channels, int zs0, int zs1,
-                        size_t vol_channel_stride, int vol_z_origin, float *partial, int nsplit, cudaStream_t st)
+                        size_t vol_channel_stride, int vol_z_origin, float *partial, int nsplit, cudaStream_t st,
+                        int mirror_z_origin)
 {
+    const bool pair = mirror_z_origin != CBCT_NO_MIRROR_PAIR;
+    if (pair && (!g->sym_mirror_z || zs1 > (g->d.vol_nz + 1) / 2)) return CBCT_ERR_INVALID_ARG;
     if (zs0 != 0 || zs1 != g->d.vol_nz || vol_z_origin != 0) { partial = nullptr; nsplit = 1; }
     const cbct_geom_desc &d = g->d;
     const double h = d.vox_mm;
@@ -421,10 +428,11 @@ int cbct_launch_adjoint(cbct_geom *g, const float *sino_src, float *vol, int cha
     G.tz = (float)(vmax / G.sdd);
     G.nu = d.det_nu; G.nv = d.det_nv; G.nx = d.vol_nx; G.ny = d.vol_ny; G.nz = d.vol_nz;
     const int NR = g->sym_rot;
-    const bool mirror = g->sym_mirror_z && zs0 == 0 && zs1 == d.vol_nz && d.vol_nz > 1;
+    const bool mirror = pair || (g->sym_mirror_z && zs0 == 0 && zs1 == d.vol_nz && d.vol_nz > 1);
     G.bx = NR == 4 ? d.vol_nx / 2 : d.vol_nx;
     G.by = NR >= 2 ? d.vol_ny / 2 : d.vol_ny;
-    G.bz0 = zs0; G.bz1 = mirror ? (d.vol_nz + 1) / 2 : zs1;
+    G.bz0 = zs0; G.bz1 = pair ? zs1 : (mirror ? (d.vol_nz + 1) / 2 : zs1);
+    G.mz_origin = pair ? mirror_z_origin : vol_z_origin;
     G.nq = 0;
     const size_t sstride = (size_t)d.n_views * d.det_nv * d.det_nu;
     if (NR == 4) {

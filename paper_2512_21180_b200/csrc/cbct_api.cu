@@ -260,18 +260,59 @@ extern "C" int cbct_fp_residual(const cbct_geom *gc, const float *vol, const flo
 // (two buffers of all channels under max_workset_bytes; D2H copies on the copy
 // stream overlap the next slab's kernel).
 // ---------------------------------------------------------------------------
+// `pairs` (the launch can fill a slab of the lower half of the grid together with its mirror image, which shares
+// all its weights): slabs then cover [z0, z1) below the middle plane plus [nz - z1, nz - z0), staged back to back.
 template <class Launch>
-static int produce_volume(CallCtx &cx, float *vol, Launch launch)
+static int produce_volume(CallCtx &cx, float *vol, bool pairs, Launch launch)
 {
     cbct_geom *g = cx.g;
     cudaStream_t st = cx.st;
     const int nz = g->d.vol_nz;
-    if (cx.kv == MEM_DEVICE) return launch(vol, 0, nz, cx.nvol, 0);
+    if (cx.kv == MEM_DEVICE) return launch(vol, 0, nz, cx.nvol, 0, CBCT_NO_MIRROR_PAIR);
     const uint64_t cap = g->d.max_workset_bytes;
     const uint64_t plane_bytes = (uint64_t)cx.plane * sizeof(float) * (uint64_t)cx.channels;
     int planes = nz;
     if (cap != 0 && plane_bytes * (uint64_t)nz > cap) planes = (int)(cap / (2 * plane_bytes));
     if (planes < 1) return CBCT_ERR_NOMEM;
+    if (pairs && planes >= 2 && nz > 1) {
+        const int nh = (nz + 1) / 2;
+        const int hp = planes >= nz ? nh : planes / 2;  // planes of the lower half per slab
+        const int n_slabs = (nh + hp - 1) / hp;
+        const int nbuf = n_slabs > 1 ? 2 : 1;
+        const size_t slab_elems = cx.plane * 2 * hp * cx.channels;
+        int rc = ensure(&g->ws_vol, &g->ws_vol_bytes, slab_elems * nbuf * sizeof(float));
+        if (rc) return rc;
+        for (int s = 0; s < n_slabs; ++s) {
+            const int b = s & 1;
+            const int z0 = s * hp, z1 = z0 + hp < nh ? z0 + hp : nh, n = z1 - z0;
+            const int mlo = nz - z1;                    // mirror images: planes [mlo, nz - z0)
+            const int skip = mlo < z1 ? z1 - mlo : 0;   // odd nz: the middle plane is its own image
+            float *buf = g->ws_vol + (size_t)b * slab_elems;
+            const size_t bstride = cx.plane * 2 * n;
+            if (s >= 2) CBCT_CUDA_TRY(cudaStreamWaitEvent(st, g->ev[b], 0));  // buffer drained by its copies
+            rc = launch(buf, z0, z1, bstride, z0, mlo - n);
+            if (rc) return rc;
+            cudaStream_t cs = n_slabs > 1 ? g->copy_stream : st;
+            if (n_slabs > 1) {
+                CBCT_CUDA_TRY(cudaEventRecord(g->ev[2 + b], st));
+                CBCT_CUDA_TRY(cudaStreamWaitEvent(cs, g->ev[2 + b], 0));
+            }
+            for (int c = 0; c < cx.channels; ++c) {
+                CBCT_CUDA_TRY(cudaMemcpyAsync(vol + c * cx.nvol + (size_t)z0 * cx.plane, buf + c * bstride,
+                                              cx.plane * n * sizeof(float), cudaMemcpyDeviceToHost, cs));
+                if (n > skip)
+                    CBCT_CUDA_TRY(cudaMemcpyAsync(vol + c * cx.nvol + (size_t)(mlo + skip) * cx.plane,
+                                                  buf + c * bstride + cx.plane * (n + skip),
+                                                  cx.plane * (n - skip) * sizeof(float), cudaMemcpyDeviceToHost, cs));
+            }
+            if (n_slabs > 1) CBCT_CUDA_TRY(cudaEventRecord(g->ev[b], cs));
+        }
+        if (n_slabs > 1) {  // join the copy stream back into `st`
+            CBCT_CUDA_TRY(cudaStreamWaitEvent(st, g->ev[0], 0));
+            CBCT_CUDA_TRY(cudaStreamWaitEvent(st, g->ev[1], 0));
+        }
+        return CBCT_OK;
+    }
     const int n_slabs = (nz + planes - 1) / planes;
     const int nbuf = n_slabs > 1 ? 2 : 1;
     const size_t slab_elems = cx.plane * planes * cx.channels;
@@ -283,7 +324,7 @@ static int produce_volume(CallCtx &cx, float *vol, Launch launch)
         float *buf = g->ws_vol + (size_t)b * slab_elems;
         const size_t bstride = cx.plane * (z1 - z0);
         if (s >= 2) CBCT_CUDA_TRY(cudaStreamWaitEvent(st, g->ev[b], 0));  // buffer drained by its copy
-        rc = launch(buf, z0, z1, bstride, z0);
+        rc = launch(buf, z0, z1, bstride, z0, CBCT_NO_MIRROR_PAIR);
         if (rc) return rc;
         cudaStream_t cs = n_slabs > 1 ? g->copy_stream : st;
         if (n_slabs > 1) {
@@ -352,8 +393,8 @@ static int adjoint_impl(const cbct_geom *gc, const float *sino, float *vol, int3
         if (rc) return rc;
         partial = g->ws_vol;
     }
-    rc = produce_volume(cx, vol, [&](float *dst, int zs0, int zs1, size_t cstride, int z_origin) {
-        return cbct_launch_adjoint(g, d_sino, dst, channels, zs0, zs1, cstride, z_origin, partial, nsplit, st);
+    rc = produce_volume(cx, vol, g->sym_mirror_z != 0, [&](float *dst, int zs0, int zs1, size_t cstride, int z_origin, int mirror_origin) {
+        return cbct_launch_adjoint(g, d_sino, dst, channels, zs0, zs1, cstride, z_origin, partial, nsplit, st, mirror_origin);
     });
     if (rc) return rc;
     if (cx.pageable) CBCT_CUDA_TRY(cudaStreamSynchronize(st));
@@ -401,7 +442,7 @@ extern "C" int cbct_bp_fdk(const cbct_geom *gc, const float *sino, float *vol, i
     rc = cbct_launch_pad_sino(g, d_sino, g->ws_sino2, channels, st);
     if (rc) return rc;
     const float *padded = g->ws_sino2;
-    rc = produce_volume(cx, vol, [&](float *dst, int zs0, int zs1, size_t cstride, int z_origin) {
+    rc = produce_volume(cx, vol, false, [&](float *dst, int zs0, int zs1, size_t cstride, int z_origin, int) {
         return cbct_launch_fdk(g, padded, dst, channels, zs0, zs1, cstride, z_origin, st);
     });
     if (rc) return rc;

@@ -21,6 +21,7 @@
 // (jx & ~7) | ((jx + CBCT_SWIZZLE_Y jy + CBCT_SWIZZLE_Z jz) & 7) of its row (cbct_fp.cu)
 #define CBCT_SWIZZLE_Y 6
 #define CBCT_SWIZZLE_Z 4
+#define CBCT_NO_MIRROR_PAIR (-2147483647 - 1)
 #define CBCT_ROW_SKEW 8          // extra cells per row of the channel-interleaved (skewed) layout (cbct_fp.cu)
 
 // View-independent geometry in voxel units (fp64), passed by value to kernels.
@@ -119,7 +120,8 @@ int cbct_launch_negate(cbct_geom *g, float *buf, size_t n, cudaStream_t st);  //
 int cbct_launch_redundancy_weight(cbct_geom *g, const float *in, float *out, int channels, cudaStream_t st);
 // gather adjoint into vol planes [zs0, zs1)
 int cbct_launch_adjoint(cbct_geom *g, const float *sino_src, float *vol, int channels, int zs0, int zs1,
-                        size_t vol_channel_stride, int vol_z_origin, float *partial, int nsplit, cudaStream_t st);
+                        size_t vol_channel_stride, int vol_z_origin, float *partial, int nsplit, cudaStream_t st,
+                        int mirror_z_origin = CBCT_NO_MIRROR_PAIR);
 int cbct_adjoint_view_splits(const cbct_geom *g);  // view groups for small grids (1 = none)
 int cbct_launch_pad_sino(cbct_geom *g, const float *src, float *dst, int channels, cudaStream_t st);
 // FDK backprojection from the padded sinogram into vol planes [zs0, zs1)
