@@ -442,8 +442,8 @@ extern "C" int cbct_bp_fdk(const cbct_geom *gc, const float *sino, float *vol, i
     rc = cbct_launch_pad_sino(g, d_sino, g->ws_sino2, channels, st);
     if (rc) return rc;
     const float *padded = g->ws_sino2;
-    rc = produce_volume(cx, vol, false, [&](float *dst, int zs0, int zs1, size_t cstride, int z_origin, int) {
-        return cbct_launch_fdk(g, padded, dst, channels, zs0, zs1, cstride, z_origin, st);
+    rc = produce_volume(cx, vol, g->sym_mirror_z != 0, [&](float *dst, int zs0, int zs1, size_t cstride, int z_origin, int mirror_origin) {
+        return cbct_launch_fdk(g, padded, dst, channels, zs0, zs1, cstride, z_origin, st, mirror_origin);
     });
     if (rc) return rc;
     if (cx.pageable) CBCT_CUDA_TRY(cudaStreamSynchronize(st));

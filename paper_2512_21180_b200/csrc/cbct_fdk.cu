@@ -178,7 +178,7 @@ fdk_kernel(const float *__restrict__ sinoP, float *__restrict__ vol, const __gri
                 } else if (NR == 2 && r == 1) {
                     x = G.nx - 1 - ix; y = G.ny - 1 - iy;
                 }
-                float *dst = vol + ((size_t)(z - vol_z_origin) * G.ny + y) * G.nx + x;
+                float *dst = vol + ((size_t)(z - (m == 0 ? vol_z_origin : G.mz_origin)) * G.ny + y) * G.nx + x;
                 *dst = accumulate ? *dst + acc[m][k][r] : acc[m][k][r];
             }
         }
@@ -230,10 +230,13 @@ static int launch_fdk(cbct_geom *g, FdkGeom &G, const float *padded, float *vol,
 // `padded_sino` is the output of cbct_launch_pad_sino.  Writes planes [zs0, zs1) of vol
 // (whose first stored plane is vol_z_origin); the z-mirror is used only when the
 // launch covers the whole grid.
+// mirror_z_origin != CBCT_NO_MIRROR_PAIR: as for cbct_launch_adjoint (a slab of the lower half plus its image).
 int cbct_launch_fdk(cbct_geom *g, const float *padded_sino, float *vol, int channels, int zs0, int zs1,
-                    size_t vol_channel_stride, int vol_z_origin, cudaStream_t st)
+                    size_t vol_channel_stride, int vol_z_origin, cudaStream_t st, int mirror_z_origin)
 {
     const cbct_geom_desc &d = g->d;
+    const bool pair = mirror_z_origin != CBCT_NO_MIRROR_PAIR;
+    if (pair && (!g->sym_mirror_z || zs1 > (d.vol_nz + 1) / 2)) return CBCT_ERR_INVALID_ARG;
     const double h = d.vox_mm;
     FdkGeom G;
     G.sid = d.sid_mm / h;
@@ -250,10 +253,11 @@ int cbct_launch_fdk(cbct_geom *g, const float *padded_sino, float *vol, int chan
     G.pu = cbct_padded_sino_pitch(g);
     G.pv = cbct_padded_sino_rows(g);
     const int NR = g->sym_rot;
-    const bool mirror = g->sym_mirror_z && zs0 == 0 && zs1 == d.vol_nz && d.vol_nz > 1;
+    const bool mirror = pair || (g->sym_mirror_z && zs0 == 0 && zs1 == d.vol_nz && d.vol_nz > 1);
     G.bx = NR == 4 ? d.vol_nx / 2 : d.vol_nx;
     G.by = NR >= 2 ? d.vol_ny / 2 : d.vol_ny;
-    G.bz0 = zs0; G.bz1 = mirror ? (d.vol_nz + 1) / 2 : zs1;
+    G.bz0 = zs0; G.bz1 = pair ? zs1 : (mirror ? (d.vol_nz + 1) / 2 : zs1);
+    G.mz_origin = pair ? mirror_z_origin : vol_z_origin;
     G.n_views = 0; G.nbase = 0;
     const size_t vs = vol_channel_stride;
     // z per thread: 3 measured best for the 8-voxel variant (1: 6.3 ms, 2: 4.8, 3: 4.6, 4: 5.2, 8: 5.3 per channel)

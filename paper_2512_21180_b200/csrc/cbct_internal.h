@@ -50,6 +50,7 @@ struct FdkGeom {
     int nx, ny, nz;
     int bx, by;             // base columns: ix < bx, iy < by (a quadrant / half if views rotate)
     int bz0, bz1;           // base planes [bz0, bz1) (the lower half if the z-mirror is used)
+    int mz_origin;          // first stored plane of the z-mirrored voxels' output (NM = 2)
     int pu, pv;             // padded sinogram pitch / rows
     int n_views;            // views in this launch
     int nbase;              // n_views_total / sym_rot
@@ -126,4 +127,5 @@ int cbct_adjoint_view_splits(const cbct_geom *g);  // view groups for small grid
 int cbct_launch_pad_sino(cbct_geom *g, const float *src, float *dst, int channels, cudaStream_t st);
 // FDK backprojection from the padded sinogram into vol planes [zs0, zs1)
 int cbct_launch_fdk(cbct_geom *g, const float *padded_sino, float *vol, int channels, int zs0, int zs1,
-                    size_t vol_channel_stride, int vol_z_origin, cudaStream_t st);
+                    size_t vol_channel_stride, int vol_z_origin, cudaStream_t st,
+                    int mirror_z_origin = CBCT_NO_MIRROR_PAIR);

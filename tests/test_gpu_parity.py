@@ -653,8 +653,8 @@ def test_fp_channel_groups(cbct, oracle_mod, C, cap, over):
 
 
 @pytest.mark.parametrize("nz,C", [(21, 1), (40, 5), (7, 2)])
-def test_streamed_adjoint_mirror_pairs(cbct, oracle_mod, nz, C):
-    """A5 + z-mirror: with a work-set cap and a HOST volume the adjoint fills each slab of the lower half together
+def test_streamed_backprojectors_mirror_pairs(cbct, oracle_mod, nz, C):
+    """A5 + z-mirror: with a work-set cap and a HOST volume the adjoint and the FDK backprojector fill each slab of the lower half together
     with its mirror image (same weights); odd nz has a middle plane that is its own image.  Against the oracle
     and, bit for bit, the resident path."""
     kw = dict(synth.geom_kwargs(synth.CONFIGS["tiny"]))
@@ -676,3 +676,9 @@ def test_streamed_adjoint_mirror_pairs(cbct, oracle_mod, nz, C):
         assert np.array_equal(out_h.numpy(), out_d.cpu().numpy())
     else:
         assert rel_l2(out_h.numpy().astype(np.float64), out_d.cpu().numpy().astype(np.float64)) <= 1e-6
+    out_h.fill_(float("nan"))
+    g.bp_fdk(dev(sino), out_h, C)
+    g0.bp_fdk(dev(sino), out_d, C)
+    torch.cuda.synchronize()
+    assert rel_l2(out_h.numpy().astype(np.float64), oracle_mod.bp_fdk(og, sino.astype(np.float64))) <= 1e-5
+    assert np.array_equal(out_h.numpy(), out_d.cpu().numpy())
