@@ -682,3 +682,25 @@ def test_streamed_backprojectors_mirror_pairs(cbct, oracle_mod, nz, C):
     torch.cuda.synchronize()
     assert rel_l2(out_h.numpy().astype(np.float64), oracle_mod.bp_fdk(og, sino.astype(np.float64))) <= 1e-5
     assert np.array_equal(out_h.numpy(), out_d.cpu().numpy())
+
+
+@pytest.mark.parametrize("C,nz", [(1, 128), (3, 129)])
+def test_adjoint_two_planes_per_thread(cbct, oracle_mod, C, nz):
+    """Grids of 2^23 voxels or more with fewer than 4 channels take the adjoint variant in which a thread owns two
+    consecutive planes (shared horizontal weights).  256 x 256 x nz voxels of 0.5 mm under the tiny detector: the
+    whole volume against the oracle (odd nz: the last thread of a column owns one plane and the middle plane is
+    its own mirror image)."""
+    kw = dict(synth.geom_kwargs(synth.CONFIGS["tiny"]))
+    kw.update(vol_nx=256, vol_ny=256, vol_nz=nz, vox_mm=0.5, n_views=8)
+    g = cbct.Geometry(**kw)
+    og = oracle_mod.Geom(**kw)
+    rng = np.random.default_rng(90 + C)
+    sino = rng.random((C,) + g.sino_shape, dtype=np.float32)
+    got = run_adj(cbct, kw, sino)
+    ref = oracle_mod.bp_adjoint(og, sino.astype(np.float64))
+    assert np.abs(ref).max() > 0
+    assert rel_l2(got, ref) <= 1e-4
+    # the same sinogram as 4 equal channels takes the one-plane-per-thread kernel: the two variants evaluate the
+    # same weights (this geometry is 3072 voxels deep, where the fp32 weights themselves are good to 5e-5)
+    four = run_adj(cbct, kw, np.repeat(sino[:1], 4, axis=0))
+    assert np.max(np.abs(got[0] - four[0])) <= 2e-6 * np.max(np.abs(ref))
