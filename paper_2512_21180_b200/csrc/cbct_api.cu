@@ -187,7 +187,7 @@ static int fp_impl(const cbct_geom *gc, const float *vol, const float *y, float 
     const RayGeom rmax = cbct_make_raygeom(g, 0, planes);
     // float4 cells per buffer: channel-interleaved groups of 4, then quad-packed channels (cbct_fp.cu)
     const size_t slab_cells = (size_t)(channels / 4) * (size_t)(rmax.px + CBCT_ROW_SKEW) * rmax.py * rmax.pz
-                              + (size_t)(channels % 4) * cbct_packed_volume_cells(rmax);
+                              + (size_t)(channels % 4) * cbct_packed_tail_cells(g, rmax);
     rc = ensure(&g->ws_vol, &g->ws_vol_bytes, slab_cells * nbuf * sizeof(float4));
     if (rc) return rc;
     const size_t stage_elems = cx.plane * planes * channels;

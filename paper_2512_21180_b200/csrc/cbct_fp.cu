@@ -100,6 +100,37 @@ pack_volume4_kernel(const float *__restrict__ src, float4 *__restrict__ dst, con
     }
 }
 
+// The same layout filled with the four quarter-turn images of ONE channel: component r of cell (x, y) is
+// f(R_r(x, y)) with R_1(x, y) = (n - 1 - y, x), R_2 = (n - 1 - x, n - 1 - y), R_3 = (y, n - 1 - x).  On a centred
+// square grid with equispaced views (cbct_geom::sym_rot == 4) the ray of view i + r n/4 through f is the ray of
+// view i through f o R_r, so projecting this cell volume over the first n/4 views yields, in its four components,
+// views i, i + n/4, i + n/2, i + 3n/4 of the channel: a single channel gets the speed of the 4-channel kernel.
+__global__ void __launch_bounds__(256)
+pack_volume_rot4_kernel(const float *__restrict__ src, float4 *__restrict__ dst, const __grid_constant__ RayGeom G,
+                        size_t src_cstride, int src_z_origin, size_t dst_cstride)
+{
+    const float *s = src + (size_t)blockIdx.z * src_cstride;
+    float4 *d = dst + (size_t)blockIdx.z * dst_cstride;
+    const int pitch = G.px + CBCT_ROW_SKEW;
+    const int pos = blockIdx.x * blockDim.x + threadIdx.x;
+    if (pos >= pitch) return;
+    const int n1 = G.nx - 1;
+    for (int row = blockIdx.y; row < G.py * G.pz; row += gridDim.y) {
+        const int jy = row % G.py, jz = row / G.py;
+        const int x = pos - ((CBCT_SWIZZLE_Y * jy + CBCT_SWIZZLE_Z * jz) & 7) - CBCT_PAD;
+        const int y = jy - CBCT_PAD, z = jz - CBCT_PAD + G.z0;
+        float4 q = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (x >= 0 && x < G.nx && y >= 0 && y < G.ny && z >= G.z0 && z < G.z1) {
+            const float *pl = s + (size_t)(z - src_z_origin) * G.ny * G.nx;
+            q.x = __ldg(pl + (size_t)y * G.nx + x);
+            q.y = __ldg(pl + (size_t)x * G.nx + (n1 - y));
+            q.z = __ldg(pl + (size_t)(n1 - y) * G.nx + (n1 - x));
+            q.w = __ldg(pl + (size_t)(n1 - x) * G.nx + y);
+        }
+        d[(size_t)row * pitch + pos] = q;
+    }
+}
+
 // ---------------------------------------------------------------------------
 // forward kernel
 // ---------------------------------------------------------------------------
@@ -284,6 +315,12 @@ size_t cbct_packed_volume_cells(const RayGeom &r) { return (size_t)r.px * r.py *
 // Layout of a packed slab of `channels` channels: channels / 4 channel-interleaved groups first, then the
 // remaining channels quad-packed one by one.  Never more than channels * cbct_packed_volume_cells(r) cells.
 static size_t packed_tail_offset(const RayGeom &r, int channels) { return (size_t)(channels / 4) * cbct_packed4_cells(r); }
+// channels left over by the groups of 4: their quarter-turn images when the geometry has that symmetry
+static bool tail_by_rotation(const cbct_geom *g, const RayGeom &r) { return g->sym_rot == 4 && r.nx == r.ny; }
+size_t cbct_packed_tail_cells(const cbct_geom *g, const RayGeom &r)
+{
+    return tail_by_rotation(g, r) ? cbct_packed4_cells(r) : cbct_packed_volume_cells(r);
+}
 
 int cbct_launch_pack_volume(cbct_geom *g, const RayGeom &r, const float *src, float4 *dst, int channels,
                             size_t src_channel_stride, int src_z_origin, cudaStream_t st)
@@ -296,6 +333,13 @@ int cbct_launch_pack_volume(cbct_geom *g, const RayGeom &r, const float *src, fl
                                                   cbct_packed4_cells(r));
         int rc = cbct_check_launch(g, "pack_volume4_kernel");
         if (rc) return rc;
+    }
+    if (tail && tail_by_rotation(g, r)) {
+        dim3 grid((r.px + CBCT_ROW_SKEW + 255) / 256, gy, tail);
+        pack_volume_rot4_kernel<<<grid, 256, 0, st>>>(src + (size_t)4 * groups * src_channel_stride,
+                                                      dst + packed_tail_offset(r, channels), r, src_channel_stride,
+                                                      src_z_origin, cbct_packed4_cells(r));
+        return cbct_check_launch(g, "pack_volume_rot4_kernel");
     }
     if (tail) {
         dim3 grid((r.px + 255) / 256, gy, tail);
@@ -361,6 +405,26 @@ int cbct_launch_fp(cbct_geom *g, const RayGeom &r, const float4 *packed, float *
         nbands = iv_hi / FP_CTA_V - band0 + 1;
     }
     ViewChunk vc;  // 8 KB; copied into the launch's parameter buffer at launch time
+    const int groups = channels / 4;
+    const bool rot_tail = channels > 4 * groups && tail_by_rotation(g, r);
+    if (rot_tail) {
+        // leftover channels one by one: the first n/4 views of the quarter-turn cell volume; the kernel's four
+        // "channels" are views i + r n/4, i.e. a channel stride of n/4 views
+        const int nbase = g->d.n_views / 4;
+        const size_t vstride = (size_t)nbase * r.nv * r.nu;
+        for (int view0 = 0; view0 < nbase; view0 += CBCT_VIEWS_PER_LAUNCH) {
+            int n = nbase - view0;
+            if (n > CBCT_VIEWS_PER_LAUNCH) n = CBCT_VIEWS_PER_LAUNCH;
+            for (int i = 0; i < n; ++i) vc.cs[i] = make_double2(g->cosphi[view0 + i], g->sinphi[view0 + i]);
+            for (int c = 4 * groups; c < channels; ++c) {
+                int rc = launch_fp4(g, r, vc, n, view0,
+                                    packed + packed_tail_offset(r, channels) + (size_t)(c - 4 * groups) * cbct_packed4_cells(r),
+                                    sino + c * sstride, accumulate, vstride, band0, nbands, sub ? sub + c * sstride : nullptr, st);
+                if (rc) return rc;
+            }
+        }
+        if (groups == 0) return CBCT_OK;
+    }
     for (int view0 = 0; view0 < g->d.n_views; view0 += CBCT_VIEWS_PER_LAUNCH) {
         int n = g->d.n_views - view0;
         if (n > CBCT_VIEWS_PER_LAUNCH) n = CBCT_VIEWS_PER_LAUNCH;
@@ -372,7 +436,7 @@ int cbct_launch_fp(cbct_geom *g, const RayGeom &r, const float4 *packed, float *
             if (rc) return rc;
         }
         const float4 *tail = packed + packed_tail_offset(r, channels) - (size_t)c * pstride;
-        while (c < channels) {
+        while (c < channels && !rot_tail) {
             int left = channels - c, rc;
             const float4 *p = tail + c * pstride;
             float *s = sino + c * sstride;

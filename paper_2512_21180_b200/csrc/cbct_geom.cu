@@ -215,9 +215,10 @@ int cbct_plan_slab_planes(const cbct_geom *g, int channels)
 {
     RayGeom r = cbct_make_raygeom(g, 0, g->d.vol_nz);
     uint64_t cap = g->d.max_workset_bytes;
-    // groups of 4 channels share one channel-interleaved cell per voxel (row pitch px + 8), the rest are quad-packed
+    // groups of 4 channels share one channel-interleaved cell per voxel (row pitch px + 8); the rest are quad-packed
+    // or, with the quarter-turn symmetry, stored as cells of their four rotated images (cbct_fp.cu)
     uint64_t packed_plane = (uint64_t)(channels / 4) * (uint64_t)(r.px + CBCT_ROW_SKEW) * r.py * 16u
-                            + (uint64_t)(channels % 4) * (uint64_t)r.px * r.py * 16u;
+                            + (uint64_t)(channels % 4) * (uint64_t)(g->sym_rot == 4 && r.nx == r.ny ? r.px + CBCT_ROW_SKEW : r.px) * r.py * 16u;
     uint64_t raw_plane = (uint64_t)r.nx * r.ny * 4u * (uint64_t)channels;
     if (cap == 0 || packed_plane * (uint64_t)r.pz + raw_plane * (uint64_t)r.nz <= cap) return g->d.vol_nz;
     int64_t planes = ((int64_t)(cap / 2) - (int64_t)(packed_plane * 2 * CBCT_PAD)) / (int64_t)(packed_plane + raw_plane);

@@ -96,6 +96,7 @@ void cbct_set_cuda_error(cudaError_t e, const char *what);
 // --- geometry helpers (cbct_geom.cu) ---------------------------------------
 RayGeom cbct_make_raygeom(const cbct_geom *g, int z0, int z1);
 size_t cbct_packed_volume_cells(const RayGeom &r);  // float4 cells per channel of a quad-packed slab
+size_t cbct_packed_tail_cells(const cbct_geom *g, const RayGeom &r);  // ... per channel left over by the groups of 4
 int cbct_padded_sino_pitch(const cbct_geom *g);
 int cbct_padded_sino_rows(const cbct_geom *g);
 int cbct_plan_slab_planes(const cbct_geom *g, int channels);  // planes per z-slab, <1 = cap too small

@@ -77,10 +77,10 @@ def test_slab_plan(cbct):
     packed, raw = 528 * 516 * 16, 4 * 512 * 512 * 4
     planes = ((1 << 30) // 2 - 4 * packed) // (packed + raw)
     assert g.num_slabs(4) == -(-512 // planes) == 9
-    # 3 channels are quad-packed (16 B per voxel and channel)
-    packed3, raw3 = 3 * 520 * 516 * 16, 3 * 512 * 512 * 4
+    # 3 channels: one 16-B cell per voxel and channel (its four quarter-turn images; this geometry has that symmetry)
+    packed3, raw3 = 3 * 528 * 516 * 16, 3 * 512 * 512 * 4
     assert g.num_slabs(3) == -(-512 // (((1 << 30) // 2 - 4 * packed3) // (packed3 + raw3)))
-    assert g.num_slabs(1) > 1  # one channel quad-packed: 520 * 516^2 * 16 B = 2.2 GB does not fit
+    assert g.num_slabs(1) > 1  # one channel in 16-B cells: 528 * 516^2 * 16 B = 2.2 GB does not fit
     assert cbct.Geometry(**kw, max_workset_bytes=3 << 30).num_slabs(1) == 1
     with pytest.raises(cbct.CbctError, match="NOMEM"):
         cbct.Geometry(**kw, max_workset_bytes=1 << 20).num_slabs(4)
