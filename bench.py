@@ -198,8 +198,14 @@ def main():
         cdist.barrier(cuda=True)
     g.profile(False)
     launches = g.launch_count() - l0
-    # groups of 4 channels go through fp4_pair_kernel, the remaining channels through fp_kernel (one timing slot)
-    fp_name = "fp_kernel" if C < 4 else ("fp4_pair_kernel" if C % 4 == 0 else "fp4_pair_kernel+fp_kernel")
+    # groups of 4 channels go through fp4_pair_kernel; so do the remaining channels (as their four quarter-turn
+    # images) when the geometry is symmetric under quarter turns, as every bench workload is: equispaced views,
+    # n_views % 4 == 0, centred square grid.  Otherwise they take the quad-packed fp_kernel (one timing slot).
+    quarter_turns = (cfg["n_views"] % 4 == 0 and cfg["vol_nx"] == cfg["vol_ny"]
+                     and cfg.get("vol_cx_mm", 0.0) == 0.0 and cfg.get("vol_cy_mm", 0.0) == 0.0
+                     and cfg.get("angles_rad") is None)
+    fp_name = ("fp4_pair_kernel" if (C % 4 == 0 or quarter_turns)
+               else ("fp_kernel" if C < 4 else "fp4_pair_kernel+fp_kernel"))
     kern = {name: g.profile_read(i) for i, name in enumerate((fp_name, "adjoint_gather_kernel", "fdk_kernel"))}
     t_fp = sum(e[0].elapsed_time(e[1]) for e in evs) / args.steps
     t_adj = sum(e[1].elapsed_time(e[2]) for e in evs) / args.steps

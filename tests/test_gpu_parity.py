@@ -365,10 +365,11 @@ def test_config5_large_streamed_sampled(cbct, oracle_mod):
     assert abs(lhs - rhs) / abs(lhs) <= 1e-5, (lhs, rhs)
 
 
-@pytest.mark.parametrize("n_views", [1040, 1037])
+@pytest.mark.parametrize("n_views", [1040, 1037, 2056])
 def test_more_views_than_one_launch_chunk(cbct, oracle_mod, n_views):
     """> 512 views: the kernels take the views in chunks of 512 and accumulate (with 1040 views the
-    rotation-shared backprojectors cross two quarter-turn blocks inside a chunk; 1037 has no rotation)."""
+    rotation-shared backprojectors cross two quarter-turn blocks inside a chunk; 1037 has no rotation; with 2056
+    the forward projector's quarter-turn path, which walks n/4 = 514 base views, needs two chunks itself)."""
     kw = dict(synth.geom_kwargs(synth.CONFIGS["tiny"]))
     kw.update(n_views=n_views, vol_nx=16, vol_ny=16, vol_nz=12, det_nu=20, det_nv=18, det_du_mm=6.0, det_dv_mm=6.0,
               det_off_u_mm=9.0)
