@@ -46,6 +46,11 @@
  *     (a cudaStream_t cast to void*, NULL = legacy default stream) and the
  *     call returns without synchronising.  A handle carries mutable
  *     workspace: calls on one handle must be ordered on one stream at a time.
+ *     The workspace grows (cudaMalloc, with a device synchronisation) only
+ *     when a call needs more than any earlier call on the handle did; after
+ *     one warm-up call of the same shape, device-pointer calls issue nothing
+ *     but kernel launches and memsets on `cuda_stream`, so they may be
+ *     captured into a CUDA graph (cudaStreamBeginCapture) and replayed.
  *   - Errors: 0 on success, a negative cbct_status otherwise; nothing throws
  *     across the ABI.  There is NO CPU fallback: without a CUDA device every
  *     compute entry point returns CBCT_ERR_CUDA.

@@ -47,3 +47,46 @@ def test_gradients_are_the_matched_operators(oracle_mod):
 
     with pytest.raises(cbct.CbctError):
         autograd.project(g, torch.zeros((4, 4, 4), device="cuda"))
+
+
+def test_calls_capture_into_a_cuda_graph():
+    """After one warm-up call per entry point (workspaces allocated), device-buffer calls only enqueue work on the
+    caller's stream, so a chain of them can be captured in a CUDA graph and replayed (launch-bound small scales of
+    the multiscale scheme); the replay must reproduce the eager results bit for bit."""
+    if not torch.cuda.is_available():
+        pytest.fail("gpu-marked tests need a CUDA device (no CPU fallback exists)")
+    from paper_2512_21180_b200 import cbct
+    g = cbct.Geometry(**synth.geom_kwargs(synth.CONFIGS["tiny"]))
+    C = 5
+    gen = torch.Generator(device="cuda").manual_seed(3)
+    x = torch.rand((C,) + g.vol_shape, device="cuda", generator=gen)
+    y = torch.empty((C,) + g.sino_shape, device="cuda")
+    q, x2, x3 = torch.empty_like(y), torch.empty_like(x), torch.empty_like(x)
+
+    def chain():
+        g.fp(x, y, C)
+        g.bp_adjoint(y, x2, C)
+        g.fdk_filter(y, q, C)
+        g.bp_fdk(q, x3, C)
+
+    chain()
+    torch.cuda.synchronize()
+    ref = (y.clone(), x2.clone(), x3.clone())
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(side):
+        chain()
+    torch.cuda.current_stream().wait_stream(side)
+    for t in (y, x2, x3):
+        t.fill_(float("nan"))
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph):
+        chain()
+    graph.replay()
+    torch.cuda.synchronize()
+    for a, b in zip(ref, (y, x2, x3)):
+        assert torch.equal(a, b)
+    x.mul_(2.0)                      # new input values in the same buffers
+    graph.replay()
+    torch.cuda.synchronize()
+    assert torch.allclose(y, 2.0 * ref[0], rtol=1e-6, atol=0.0)
