@@ -1,4 +1,6 @@
-"""The autograd wrappers hand gradients to the matched pair: d<P x, y>/dx must be cbct_bp_adjoint(y) bit for bit,
+"""How the library sits in a PyTorch program: autograd, CUDA-graph capture, several handles on several streams.
+
+The autograd wrappers hand gradients to the matched pair: d<P x, y>/dx must be cbct_bp_adjoint(y) bit for bit,
 d<P^T y, x>/dy must be cbct_fp(x), and a Landweber-type loss 1/2 |P x - y|^2 must have the gradient P^T (P x - y)
 the oracle computes (Alg. 1 l.19)."""
 import numpy as np
@@ -90,3 +92,39 @@ def test_calls_capture_into_a_cuda_graph():
     graph.replay()
     torch.cuda.synchronize()
     assert torch.allclose(y, 2.0 * ref[0], rtol=1e-6, atol=0.0)
+
+
+def test_two_handles_on_two_streams():
+    """The library keeps no mutable global state: two handles (different geometries) driven concurrently on two
+    streams give the results of running them one after the other."""
+    if not torch.cuda.is_available():
+        pytest.fail("gpu-marked tests need a CUDA device (no CPU fallback exists)")
+    from paper_2512_21180_b200 import cbct
+    kws = [synth.geom_kwargs(synth.CONFIGS["tiny"]),
+           dict(synth.geom_kwargs(synth.CONFIGS["small_halffan"]), n_views=20)]
+    gs = [cbct.Geometry(**kw) for kw in kws]
+    gen = torch.Generator(device="cuda").manual_seed(5)
+    C = 3
+    xs = [torch.rand((C,) + g.vol_shape, device="cuda", generator=gen) for g in gs]
+
+    def run(g, x, stream=None):
+        y = torch.empty((C,) + g.sino_shape, device="cuda")
+        b = torch.empty_like(x)
+        f = torch.empty_like(x)
+        g.fp(x, y, C, stream=stream)
+        g.bp_adjoint(y, b, C, stream=stream)
+        g.bp_fdk(y, f, C, stream=stream)
+        return y, b, f
+
+    ref = [run(g, x) for g, x in zip(gs, xs)]
+    torch.cuda.synchronize()
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    outs = [None, None]
+    for rep in range(3):
+        for i in (0, 1):
+            with torch.cuda.stream(streams[i]):
+                outs[i] = run(gs[i], xs[i], stream=streams[i])
+    torch.cuda.synchronize()
+    for r, o in zip(ref, outs):
+        for a, b in zip(r, o):
+            assert torch.equal(a, b)
