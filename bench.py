@@ -134,6 +134,7 @@ def main():
                          "With a cap the volumes live in pinned HOST memory and stream through z-slabs")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-lire", action="store_true", help="skip the Alg. 1 operator-sequence timing (context)")
     args = ap.parse_args()
 
     from paper_2512_21180_b200 import synth
@@ -362,6 +363,10 @@ def main():
         line["next"] = next1
     if e2e:
         line["e2e"] = e2e
+    if not args.no_lire and world == 1 and cfg["name"] == "multichannel_256" and not streamed:
+        # context, outside the step: the operator calls of one LIRE++ inference (Alg. 1) at this grid and view count
+        from paper_2512_21180_b200 import lire_ops
+        line["lire_ops"] = lire_ops.measure(cfg["vol_nx"], cfg["n_views"], reps=2)
     if not args.no_cpu_baseline and world == 1:
         line["cpu_baseline"], _ = oracle_sample(cfg, 1, 0)
     print(json.dumps(line))

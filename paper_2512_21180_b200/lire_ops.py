@@ -138,33 +138,38 @@ class LireOperators:
         return outputs
 
 
+def measure(n: int = 256, views: int = 400, reps: int = 3) -> dict:
+    """One warm-up pass, then `reps` timed passes of the operator sequence on seeded uniform(0,1) projections;
+    CUDA-event time of each group of calls, averaged over the passes."""
+    if not torch.cuda.is_available():
+        raise cbct.CbctError("needs a CUDA device: there is no CPU fallback")
+    ops = LireOperators(n, views)
+    gen = torch.Generator(device="cuda").manual_seed(1234)
+    y_raw = torch.rand((views, n, n), device="cuda", generator=gen)
+    ops.reconstruct_operators(y_raw)                 # warm-up
+    torch.cuda.synchronize()
+    timings: dict = {}
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a.record()
+    for _ in range(reps):
+        ops.reconstruct_operators(y_raw, timings)
+    b.record()
+    torch.cuda.synchronize()
+    groups = {k: sum(s.elapsed_time(e) for s, e in v) / reps for k, v in timings.items()}
+    return {"what": "operator calls of one LIRE++ RECONSTRUCT (Alg. 1), learned blocks replaced by stand-ins",
+            "grid": n, "views": views, "reps": reps,
+            "ms_by_group": {k: round(v, 3) for k, v in groups.items()},
+            "ms_operators": round(sum(groups.values()), 3),
+            "ms_wall_incl_standins": round(a.elapsed_time(b) / reps, 3)}
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--n", type=int, default=256)
     ap.add_argument("--views", type=int, default=400, help="the paper evaluates at 720 (PAPER.md:139)")
     ap.add_argument("--reps", type=int, default=3)
     args = ap.parse_args()
-    if not torch.cuda.is_available():
-        raise cbct.CbctError("needs a CUDA device: there is no CPU fallback")
-    ops = LireOperators(args.n, args.views)
-    gen = torch.Generator(device="cuda").manual_seed(1234)
-    y_raw = torch.rand((args.views, args.n, args.n), device="cuda", generator=gen)
-    ops.reconstruct_operators(y_raw)                 # warm-up
-    torch.cuda.synchronize()
-    timings: dict = {}
-    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    a.record()
-    for _ in range(args.reps):
-        ops.reconstruct_operators(y_raw, timings)
-    b.record()
-    torch.cuda.synchronize()
-    groups = {k: sum(s.elapsed_time(e) for s, e in v) / args.reps for k, v in timings.items()}
-    print(json.dumps({
-        "what": "operator calls of one LIRE++ RECONSTRUCT (Alg. 1), learned blocks replaced by stand-ins",
-        "grid": args.n, "views": args.views, "reps": args.reps,
-        "ms_by_group": {k: round(v, 3) for k, v in groups.items()},
-        "ms_operators": round(sum(groups.values()), 3),
-        "ms_wall_incl_standins": round(a.elapsed_time(b) / args.reps, 3)}))
+    print(json.dumps(measure(args.n, args.views, args.reps)))
 
 
 if __name__ == "__main__":
