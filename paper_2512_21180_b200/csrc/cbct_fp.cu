@@ -177,21 +177,25 @@ __device__ __forceinline__ float quad_sample(const Sample &s, size_t off)
     return lerpf(b0, b1, s.fz);
 }
 
-// CB channels per thread; a warp covers TU x (32 / TU) pixels; CTA = 16 x 16 pixels.
+// CB channels per thread; a warp covers TU x (32 / TU) pixels; CTA = FPK_VPC consecutive views x (16 pixels in u x
+// one row of warps), see fp4_pair_kernel for why a CTA spans views.
+#ifndef FPK_VPC
+#define FPK_VPC 4
+#endif
 template <int CB, int TU>
-__global__ void __launch_bounds__(FP_CTA_U *FP_CTA_V)
+__global__ void __launch_bounds__(32 * (FP_CTA_U / TU) * FPK_VPC)
 fp_kernel(const float4 *__restrict__ packed, float *__restrict__ sino, const __grid_constant__ RayGeom G,
           const __grid_constant__ ViewChunk V, int view0, int accumulate, size_t packed_cstride,
-          size_t sino_cstride, int band0, const float *__restrict__ sub)
+          size_t sino_cstride, int band0, const float *__restrict__ sub, int nviews)
 {
     constexpr int TV = 32 / TU, WU = FP_CTA_U / TU;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int iu = blockIdx.x * FP_CTA_U + (warp % WU) * TU + (lane % TU);
     // grid = (u tiles, views, v bands): CTAs in flight share a band of detector rows, i.e. a thin
     // z-slab of the volume, which then stays L2-resident across all views
-    const int iv = (band0 + blockIdx.z) * FP_CTA_V + (warp / WU) * TV + (lane / TU);
-    if (iu >= G.nu || iv >= G.nv) return;
-    const int view = blockIdx.y;
+    const int iv = (band0 + blockIdx.z) * TV + (lane / TU);
+    const int view = blockIdx.y * FPK_VPC + warp / WU;
+    if (iu >= G.nu || iv >= G.nv || view >= nviews) return;
     const Ray r = cbct_ray_setup(G, V.cs[view].x, V.cs[view].y, iu, iv);
     const unsigned py = G.py, px = G.px, plane = G.px * G.py;
     const unsigned kfold = (CBCT_MAGIC_BITS * (py + 1u)) * px;  // magic bits of jz, jy folded through the row formula
@@ -371,16 +375,20 @@ static int launch_fp_cb(cbct_geom *g, const RayGeom &r, const ViewChunk &vc, int
                         const float4 *packed, float *sino, int accumulate, size_t pstride, size_t sstride,
                         int band0, int nbands, const float *sub, cudaStream_t st)
 {
-    dim3 grid((r.nu + FP_CTA_U - 1) / FP_CTA_U, nviews, nbands);
+    // the caller counts bands of FP_CTA_V = 16 rows; a CTA covers one row of warps, 32 / TU detector rows
+    dim3 grid((r.nu + FP_CTA_U - 1) / FP_CTA_U, (nviews + FPK_VPC - 1) / FPK_VPC, 0);
     cbct_prof_begin(g, CBCT_KERNEL_FP, st);
     // 4 x 8-pixel warps suit the bank swizzle best when rays cross the whole volume; in a thin z-slab
     // (streaming) 8 x 4-pixel warps keep the lanes' in-slab segments alike (measured on config 5: +17 %)
-    if (r.z1 - r.z0 >= 64 || r.z1 - r.z0 == r.nz)
-        fp_kernel<CB, 4><<<grid, FP_CTA_U * FP_CTA_V, 0, st>>>(packed, sino, r, vc, view0, accumulate, pstride, sstride,
-                                                               band0, sub);
-    else
-        fp_kernel<CB, 8><<<grid, FP_CTA_U * FP_CTA_V, 0, st>>>(packed, sino, r, vc, view0, accumulate, pstride, sstride,
-                                                               band0, sub);
+    if (r.z1 - r.z0 >= 64 || r.z1 - r.z0 == r.nz) {
+        grid.z = nbands * (FP_CTA_V / 8);
+        fp_kernel<CB, 4><<<grid, 32 * (FP_CTA_U / 4) * FPK_VPC, 0, st>>>(packed, sino, r, vc, view0, accumulate, pstride,
+                                                                         sstride, band0 * (FP_CTA_V / 8), sub, nviews);
+    } else {
+        grid.z = nbands * (FP_CTA_V / 4);
+        fp_kernel<CB, 8><<<grid, 32 * (FP_CTA_U / 8) * FPK_VPC, 0, st>>>(packed, sino, r, vc, view0, accumulate, pstride,
+                                                                         sstride, band0 * (FP_CTA_V / 4), sub, nviews);
+    }
     cbct_prof_end(g, CBCT_KERNEL_FP, st);
     return cbct_check_launch(g, "fp_kernel");
 }
