@@ -30,7 +30,7 @@ UNIT = "Gsamples/s"
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of each kernel at the default workload,
 # from the ncu --set full captures summarised in profiles/r1_final.md (multichannel_256; fp and adjoint launches
 # carry 4 channels, fdk launches 1).  Reported only for that workload.
-NCU_DRAM_BYTES_PER_LAUNCH = {"fp4_pair_kernel": 0.579e9, "adjoint_gather_kernel": 0.278e9, "fdk_kernel": 0.209e9}
+NCU_DRAM_BYTES_PER_LAUNCH = {"fp4_pair_kernel": 0.579e9, "adjoint_gather_kernel": 7.39e9, "fdk_kernel": 0.209e9}
 
 
 def peaks():
