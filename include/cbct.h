@@ -46,11 +46,22 @@
  *     (a cudaStream_t cast to void*, NULL = legacy default stream) and the
  *     call returns without synchronising.  A handle carries mutable
  *     workspace: calls on one handle must be ordered on one stream at a time.
- *     The workspace grows (cudaMalloc, with a device synchronisation) only
- *     when a call needs more than any earlier call on the handle did; after
- *     one warm-up call of the same shape, device-pointer calls issue nothing
- *     but kernel launches and memsets on `cuda_stream`, so they may be
- *     captured into a CUDA graph (cudaStreamBeginCapture) and replayed.
+ *     The workspace grows (cudaFree + cudaMalloc, with a device
+ *     synchronisation) only when a call needs more than any earlier call on
+ *     the handle did; after one warm-up call of the same shape -- or
+ *     cbct_geom_reserve -- device-pointer calls issue nothing but kernel
+ *     launches and memsets on `cuda_stream`, so they may be captured into a
+ *     CUDA graph (cudaStreamBeginCapture) and replayed.  A captured graph
+ *     bakes in the workspace addresses: ANY later growth of the workspace
+ *     (a call with more channels, the first call of another operator)
+ *     invalidates graphs captured before it -- reserve for the largest call
+ *     first.  A call that would have to grow the workspace while its stream
+ *     is capturing returns CBCT_ERR_UNSUPPORTED and enqueues nothing; host
+ *     buffers are refused during capture (their staging uses side streams).
+ *   - Devices: the library launches on the CUDA device that is current in the calling thread; a handle's
+ *     workspace belongs to the device that was current at its first compute call, so use one handle per
+ *     device.  All device pointers of a call must belong to that device (the Python binding checks this and
+ *     makes the tensors' device current for the call).
  *   - Errors: 0 on success, a negative cbct_status otherwise; nothing throws
  *     across the ABI.  There is NO CPU fallback: without a CUDA device every
  *     compute entry point returns CBCT_ERR_CUDA.
@@ -93,8 +104,15 @@ typedef struct cbct_geom_desc {
     double vox_mm;                /* isotropic voxel pitch h                   2.0        */
     double vol_cx_mm, vol_cy_mm, vol_cz_mm; /* volume centre rel. to isocentre  0,0,0     */
     double step_vox;              /* ray step in voxel units, 0 < step <= 1    0.5        */
-    uint64_t max_workset_bytes;   /* 0 = no cap; else cap on device bytes holding volume
-                                     data at once => z-slab streaming (A5)               */
+    uint64_t max_workset_bytes;   /* 0 = no cap; else cap on device bytes holding VOLUME
+                                     data at once => z-slab streaming (A5).  It does not
+                                     cap the sinogram side: a call keeps the sinogram of
+                                     all its channels (when given as a host buffer) and one
+                                     re-laid-out copy of it (view-interleaved for the
+                                     adjoint, zero-bordered for FDK) resident beside the
+                                     slabs: 2 x 4 B x channels x n_views x nv x nu, e.g.
+                                     3.0 + 3.0 GB for 4 channels of 720 x 512 x 512
+                                     (cbct_geom_workspace_bytes reports the total).       */
 } cbct_geom_desc;
 
 /* A1.  Validates `d`, precomputes the per-view tables (fp64 on the host,
@@ -184,6 +202,28 @@ int cbct_geom_count_samples(const cbct_geom *g, uint64_t *out);
 /* Number of z-slabs the streaming path (A5) uses for `channels` channels
  * (1 = everything resident).  Needs no CUDA device. */
 int cbct_geom_num_slabs(const cbct_geom *g, int32_t channels, int32_t *out);
+
+/* Device bytes of workspace the handle owns right now (packed slabs / staging, sinogram copies, tables). */
+int cbct_geom_workspace_bytes(const cbct_geom *g, uint64_t *out);
+
+/* Allocates, up front, all the workspace that device-pointer calls of cbct_fp / cbct_bp_adjoint(_weighted) /
+ * cbct_bp_fdk / cbct_fdk_filter with up to `channels` channels need, so that they neither allocate nor
+ * synchronise afterwards (CUDA-graph capture; flat memory).  Synchronises the device if it has to grow. */
+int cbct_geom_reserve(cbct_geom *g, int32_t channels);
+
+/* Plane ranges of the backprojectors: the shard a rank owns when one volume is split over GPUs (SURVEY.md
+ * s.8(e) item 2: view-sharded cbct_fp, one all-gather of the sinogram, plane-sharded backprojection).
+ * DEVICE pointers.  out[c] receives planes [z0, z1) of channel c of what cbct_bp_adjoint / cbct_bp_fdk would
+ * write (the same terms; fp32 summation order, hence the last bits, may differ from the whole-volume call, which
+ * pairs planes and splits views differently on some grids).  mirror_pair != 0 (only for geometries symmetric under z -> -z: vol_cz_mm = 0,
+ * det_off_v_mm = 0; needs z1 <= ceil(nz / 2)): out[c] holds [z0, z1) followed by the mirror images
+ * [nz - z1 + skip, nz - z0) in ascending order, skip = 1 if the range contains the middle plane of an odd nz
+ * (its own image), else 0 -- 2 (z1 - z0) - skip planes per channel; the pair shares every weight, as in the
+ * whole-volume call. */
+int cbct_bp_adjoint_slab(const cbct_geom *g, const float *sino, float *out, int32_t channels, int32_t z0, int32_t z1,
+                         int32_t mirror_pair, void *cuda_stream);
+int cbct_bp_fdk_slab(const cbct_geom *g, const float *sino, float *out, int32_t channels, int32_t z0, int32_t z1,
+                     int32_t mirror_pair, void *cuda_stream);
 
 /* Kernels launched by this handle since creation (for bench.py's gpu_launches). */
 int cbct_geom_launch_count(const cbct_geom *g, uint64_t *out);

@@ -20,6 +20,7 @@ LIB_PATH = os.path.join(_HERE, "libcbct.so")
 EXPORTS = (
     "cbct_geom_create", "cbct_geom_destroy", "cbct_fp", "cbct_bp_adjoint", "cbct_bp_fdk",
     "cbct_geom_count_samples", "cbct_geom_num_slabs", "cbct_geom_launch_count",
+    "cbct_geom_workspace_bytes", "cbct_geom_reserve", "cbct_bp_adjoint_slab", "cbct_bp_fdk_slab",
     "cbct_geom_profile", "cbct_geom_profile_read",
     "cbct_fdk_filter", "cbct_redundancy_weight", "cbct_geom_redundancy_weights",
     "cbct_fp_residual", "cbct_bp_adjoint_weighted",
@@ -71,6 +72,10 @@ def load_library() -> ctypes.CDLL:
     L.cbct_geom_count_samples.argtypes = [vp, ctypes.POINTER(ctypes.c_uint64)]
     L.cbct_geom_num_slabs.argtypes = [vp, i32, ctypes.POINTER(i32)]
     L.cbct_geom_launch_count.argtypes = [vp, ctypes.POINTER(ctypes.c_uint64)]
+    L.cbct_geom_workspace_bytes.argtypes = [vp, ctypes.POINTER(ctypes.c_uint64)]
+    L.cbct_geom_reserve.argtypes = [vp, i32]
+    for name in ("cbct_bp_adjoint_slab", "cbct_bp_fdk_slab"):
+        getattr(L, name).argtypes = [vp, vp, vp, i32, i32, i32, i32, vp]
     L.cbct_geom_profile.argtypes = [vp, ctypes.c_int]
     L.cbct_geom_profile_read.argtypes = [vp, ctypes.c_int, ctypes.POINTER(ctypes.c_double),
                                          ctypes.POINTER(ctypes.c_uint64)]
@@ -121,15 +126,44 @@ def _ptr_and_keep(t, n_expected: int):
     return t.data_ptr()
 
 
-def _stream_handle(stream) -> int:
+def _stream_handle(stream, device=None) -> int:
     if stream is None:
         import torch
         if torch.cuda.is_available():
-            return int(torch.cuda.current_stream().cuda_stream)
+            return int(torch.cuda.current_stream(device).cuda_stream)
         return 0
     if isinstance(stream, int):
         return stream
     return int(stream.cuda_stream)
+
+
+class _on_device_of:
+    """Context for one C-ABI call: all CUDA tensors among `tensors` must live on ONE device; that device is made
+    current for the call (the library launches on the current device) and `self.stream` is the handle of `stream`,
+    or of torch's current stream ON THAT DEVICE.  Host tensors / numpy arrays place no constraint."""
+
+    def __init__(self, tensors, stream):
+        self.dev, self._ctx = None, None
+        for t in tensors:
+            d = getattr(t, "device", None)
+            if d is not None and getattr(d, "type", "cpu") == "cuda":
+                if self.dev is not None and d != self.dev:
+                    raise CbctError(f"tensors on different CUDA devices ({self.dev} and {d}) in one call")
+                self.dev = d
+        self._stream = stream
+
+    def __enter__(self):
+        if self.dev is not None:
+            import torch
+            self._ctx = torch.cuda.device(self.dev)
+            self._ctx.__enter__()
+        self.stream = _stream_handle(self._stream, self.dev)
+        return self
+
+    def __exit__(self, *exc):
+        if self._ctx is not None:
+            self._ctx.__exit__(*exc)
+        return False
 
 
 class Geometry:
@@ -175,33 +209,61 @@ class Geometry:
     def fp(self, vol, sino, channels: int = 1, stream=None):
         """cbct_fp: vol[C,nz,ny,nx] -> sino[C,n_views,nv,nu] (overwritten)."""
         pv, ps = _ptr_and_keep(vol, channels * self.n_vol), _ptr_and_keep(sino, channels * self.n_sino)
-        _check(load_library().cbct_fp(self._h, pv, ps, channels, _stream_handle(stream)))
+        with _on_device_of((vol, sino), stream) as cx:
+            _check(load_library().cbct_fp(self._h, pv, ps, channels, cx.stream))
         return sino
 
     def bp_adjoint(self, sino, vol, channels: int = 1, stream=None):
         """cbct_bp_adjoint: sino -> vol (overwritten), exact transpose of fp."""
         ps, pv = _ptr_and_keep(sino, channels * self.n_sino), _ptr_and_keep(vol, channels * self.n_vol)
-        _check(load_library().cbct_bp_adjoint(self._h, ps, pv, channels, _stream_handle(stream)))
+        with _on_device_of((vol, sino), stream) as cx:
+            _check(load_library().cbct_bp_adjoint(self._h, ps, pv, channels, cx.stream))
         return vol
 
     def bp_fdk(self, sino, vol, channels: int = 1, stream=None):
         """cbct_bp_fdk: FDK-weighted voxel-driven backprojection stage."""
         ps, pv = _ptr_and_keep(sino, channels * self.n_sino), _ptr_and_keep(vol, channels * self.n_vol)
-        _check(load_library().cbct_bp_fdk(self._h, ps, pv, channels, _stream_handle(stream)))
+        with _on_device_of((vol, sino), stream) as cx:
+            _check(load_library().cbct_bp_fdk(self._h, ps, pv, channels, cx.stream))
         return vol
+
+    def slab_planes(self, z0: int, z1: int, mirror_pair: bool = False) -> int:
+        """Planes per channel that bp_adjoint_slab / bp_fdk_slab write for the range [z0, z1)."""
+        n = z1 - z0
+        if not mirror_pair:
+            return n
+        nz = self.vol_shape[0]
+        return 2 * n - (1 if nz - z1 < z1 else 0)
+
+    def bp_adjoint_slab(self, sino, out, z0: int, z1: int, channels: int = 1, mirror_pair: bool = False, stream=None):
+        """cbct_bp_adjoint_slab: planes [z0, z1) (+ their z-mirror images) of bp_adjoint, device tensors."""
+        n_out = channels * self.slab_planes(z0, z1, mirror_pair) * self.vol_shape[1] * self.vol_shape[2]
+        ps, po = _ptr_and_keep(sino, channels * self.n_sino), _ptr_and_keep(out, n_out)
+        with _on_device_of((sino, out), stream) as cx:
+            _check(load_library().cbct_bp_adjoint_slab(self._h, ps, po, channels, z0, z1, 1 if mirror_pair else 0, cx.stream))
+        return out
+
+    def bp_fdk_slab(self, sino, out, z0: int, z1: int, channels: int = 1, mirror_pair: bool = False, stream=None):
+        """cbct_bp_fdk_slab: planes [z0, z1) (+ their z-mirror images) of bp_fdk, device tensors."""
+        n_out = channels * self.slab_planes(z0, z1, mirror_pair) * self.vol_shape[1] * self.vol_shape[2]
+        ps, po = _ptr_and_keep(sino, channels * self.n_sino), _ptr_and_keep(out, n_out)
+        with _on_device_of((sino, out), stream) as cx:
+            _check(load_library().cbct_bp_fdk_slab(self._h, ps, po, channels, z0, z1, 1 if mirror_pair else 0, cx.stream))
+        return out
 
     # --- NEXT-1: FDK front end ------------------------------------------------
     def fdk_filter(self, sino_in, sino_out, channels: int = 1, redundancy: bool = True, stream=None):
         """cbct_fdk_filter: weighted + ramp-filtered projections q such that bp_fdk(q) = FDK_w."""
         pi, po = _ptr_and_keep(sino_in, channels * self.n_sino), _ptr_and_keep(sino_out, channels * self.n_sino)
-        _check(load_library().cbct_fdk_filter(self._h, pi, po, channels, 1 if redundancy else 0,
-                                              _stream_handle(stream)))
+        with _on_device_of((sino_in, sino_out), stream) as cx:
+            _check(load_library().cbct_fdk_filter(self._h, pi, po, channels, 1 if redundancy else 0, cx.stream))
         return sino_out
 
     def redundancy_weight(self, sino_in, sino_out, channels: int = 1, stream=None):
         """cbct_redundancy_weight: sino_out = w(u) * sino_in (in place allowed)."""
         pi, po = _ptr_and_keep(sino_in, channels * self.n_sino), _ptr_and_keep(sino_out, channels * self.n_sino)
-        _check(load_library().cbct_redundancy_weight(self._h, pi, po, channels, _stream_handle(stream)))
+        with _on_device_of((sino_in, sino_out), stream) as cx:
+            _check(load_library().cbct_redundancy_weight(self._h, pi, po, channels, cx.stream))
         return sino_out
 
     def redundancy_weights(self) -> np.ndarray:
@@ -215,19 +277,23 @@ class Geometry:
         """cbct_fp_residual: sino = P vol - y (y: device sinogram)."""
         pv, py = _ptr_and_keep(vol, channels * self.n_vol), _ptr_and_keep(y, channels * self.n_sino)
         ps = _ptr_and_keep(sino, channels * self.n_sino)
-        _check(load_library().cbct_fp_residual(self._h, pv, py, ps, channels, _stream_handle(stream)))
+        with _on_device_of((vol, y, sino), stream) as cx:
+            _check(load_library().cbct_fp_residual(self._h, pv, py, ps, channels, cx.stream))
         return sino
 
     def bp_adjoint_weighted(self, sino, vol, channels: int = 1, stream=None):
         """cbct_bp_adjoint_weighted: vol = P^T (w(u) * sino)."""
         ps, pv = _ptr_and_keep(sino, channels * self.n_sino), _ptr_and_keep(vol, channels * self.n_vol)
-        _check(load_library().cbct_bp_adjoint_weighted(self._h, ps, pv, channels, _stream_handle(stream)))
+        with _on_device_of((sino, vol), stream) as cx:
+            _check(load_library().cbct_bp_adjoint_weighted(self._h, ps, pv, channels, cx.stream))
         return vol
 
     # --- NEXT-2: field-of-view tensor -----------------------------------------
     def fov(self, vol_out, stream=None):
         """cbct_fov: V[nz,ny,nx] = fraction of views in which each voxel is visible."""
-        _check(load_library().cbct_fov(self._h, _ptr_and_keep(vol_out, self.n_vol), _stream_handle(stream)))
+        po = _ptr_and_keep(vol_out, self.n_vol)
+        with _on_device_of((vol_out,), stream) as cx:
+            _check(load_library().cbct_fov(self._h, po, cx.stream))
         return vol_out
 
     # --- host-side queries --------------------------------------------------
@@ -240,6 +306,16 @@ class Geometry:
         out = ctypes.c_int32()
         _check(load_library().cbct_geom_num_slabs(self._h, channels, ctypes.byref(out)))
         return int(out.value)
+
+    def workspace_bytes(self) -> int:
+        """cbct_geom_workspace_bytes: device bytes of workspace the handle owns right now."""
+        out = ctypes.c_uint64()
+        _check(load_library().cbct_geom_workspace_bytes(self._h, ctypes.byref(out)))
+        return int(out.value)
+
+    def reserve(self, channels: int = 1):
+        """cbct_geom_reserve: allocate all workspace for device-pointer calls with up to `channels` channels."""
+        _check(load_library().cbct_geom_reserve(self._h, channels))
 
     def profile(self, enable: bool = True):
         """cbct_geom_profile: record a CUDA-event pair around every main-kernel launch."""
@@ -271,7 +347,8 @@ def downsample(vol_in, vol_out, factor: int, stream=None):
     o, nz, ny, nx = _shape4(vol_in)
     pi = _ptr_and_keep(vol_in, o * nz * ny * nx)
     po = _ptr_and_keep(vol_out, o * (nz // factor) * (ny // factor) * (nx // factor))
-    _check(load_library().cbct_downsample(pi, po, o, nz, ny, nx, factor, _stream_handle(stream)))
+    with _on_device_of((vol_in, vol_out), stream) as cx:
+        _check(load_library().cbct_downsample(pi, po, o, nz, ny, nx, factor, cx.stream))
     return vol_out
 
 
@@ -280,7 +357,8 @@ def upsample(vol_in, vol_out, factor: int, stream=None):
     o, nz, ny, nx = _shape4(vol_in)
     pi = _ptr_and_keep(vol_in, o * nz * ny * nx)
     po = _ptr_and_keep(vol_out, o * nz * ny * nx * factor ** 3)
-    _check(load_library().cbct_upsample(pi, po, o, nz, ny, nx, factor, _stream_handle(stream)))
+    with _on_device_of((vol_in, vol_out), stream) as cx:
+        _check(load_library().cbct_upsample(pi, po, o, nz, ny, nx, factor, cx.stream))
     return vol_out
 
 
@@ -289,7 +367,8 @@ def proj_down(sino_in, sino_out, factor: int, stream=None):
     o, nviews, nv, nu = _shape4(sino_in)
     pi = _ptr_and_keep(sino_in, o * nviews * nv * nu)
     po = _ptr_and_keep(sino_out, o * (-(-nviews // factor)) * (nv // factor) * (nu // factor))
-    _check(load_library().cbct_proj_down(pi, po, o, nviews, nv, nu, factor, _stream_handle(stream)))
+    with _on_device_of((sino_in, sino_out), stream) as cx:
+        _check(load_library().cbct_proj_down(pi, po, o, nviews, nv, nu, factor, cx.stream))
     return sino_out
 
 
@@ -298,7 +377,8 @@ def water_bone(rho_hat, rho_w, rho_b, tau0: float = 0.0, tau1: float = 1.2, tau2
     """cbct_water_bone: Eq. (3)-(4) water / bone densities of a modified-CT-number array (any shape)."""
     n = int(np.prod(rho_hat.shape))
     pr, pw, pb = (_ptr_and_keep(t, n) for t in (rho_hat, rho_w, rho_b))
-    _check(load_library().cbct_water_bone(pr, pw, pb, n, tau0, tau1, tau2, kappa_b, _stream_handle(stream)))
+    with _on_device_of((rho_hat, rho_w, rho_b), stream) as cx:
+        _check(load_library().cbct_water_bone(pr, pw, pb, n, tau0, tau1, tau2, kappa_b, cx.stream))
     return rho_w, rho_b
 
 
@@ -312,6 +392,7 @@ def polychromatic_primary(pw, pb, i0, mu_w, mu_b, resp, out, stream=None):
     pa, pb_, po = (_ptr_and_keep(t, n_views * n_pix) for t in (pw, pb, out))
     pi = _ptr_and_keep(i0, n_bins * n_pix)
     arr = [(ctypes.c_double * n_bins)(*[float(x) for x in t]) for t in (mu_w, mu_b, resp)]
-    _check(load_library().cbct_polychromatic_primary(pa, pb_, pi, arr[0], arr[1], arr[2], n_bins, n_views, n_pix, po,
-                                                     _stream_handle(stream)))
+    with _on_device_of((pw, pb, i0, out), stream) as cx:
+        _check(load_library().cbct_polychromatic_primary(pa, pb_, pi, arr[0], arr[1], arr[2], n_bins, n_views, n_pix,
+                                                         po, cx.stream))
     return out

@@ -30,6 +30,8 @@
 // W(j, i) y[i + r n/NR] into the accumulator of the r-th rotated voxel -- and
 // NM = 2 voxels mirrored in z (ray iv <-> nv-1-iv).  One weight evaluation
 // then feeds NR * NM * CB accumulators.
+#include <atomic>
+
 #include "cbct_device.cuh"
 
 struct AdjGeom {
@@ -39,6 +41,7 @@ struct AdjGeom {
     double inv_step;
     float step, scale;                      // ray step (voxel units); Delta in mm
     float tz;                               // max |v| / sdd over the detector
+    int fine;                               // the sample window of a (voxel, ray) pair can hold more than 6 lattice points
     int nu, nv, nx, ny, nz;
     int bx, by;                             // base domain: ix < bx, iy < by
     int bz0, bz1;                           // base planes [bz0, bz1)
@@ -193,14 +196,14 @@ adjoint_gather_kernel(const float *__restrict__ sinoI, float *__restrict__ vol, 
                 // the 6th only when the window reaches it); samples past the window have weight 0 (clamps)
 #pragma unroll
                 for (int j = 0; j < 6; ++j) {
-                    const float wx = fmaxf(1.0f - fabsf(ex), 0.f);
-                    const float wy = fmaxf(1.0f - fabsf(ey), 0.f);
+                    const float wx = __saturatef(1.0f - fabsf(ex));
+                    const float wy = __saturatef(1.0f - fabsf(ey));
                     if (ZT == 1) {
-                        W[0] = fmaf(wx * wy, fmaxf(1.0f - fabsf(ez), 0.f), W[0]);
+                        W[0] = fmaf(wx * wy, __saturatef(1.0f - fabsf(ez)), W[0]);
                     } else {
                         const float wxy = wx * wy;
 #pragma unroll
-                        for (int t = 0; t < ZT; ++t) W[t] = fmaf(wxy, fmaxf(1.0f - fabsf(ez - (float)t), 0.f), W[t]);
+                        for (int t = 0; t < ZT; ++t) W[t] = fmaf(wxy, __saturatef(1.0f - fabsf(ez - (float)t)), W[t]);
                     }
                     if (j == 4 && fmaf(lam_hi, invg, -5.5f) <= klo) break;  // k = klo + 5 is past the window
                     ex += gNx; ey += gNy; ez += gv;
@@ -208,9 +211,9 @@ adjoint_gather_kernel(const float *__restrict__ sinoI, float *__restrict__ vol, 
                 if (FINE) {  // steps finer than 1/2 voxel: walk the rest of the window
                     const float kend = fmaf(lam_hi, invg, -0.5f);  // samples with k < kend are inside
                     for (float kf = klo + 6.0f; kf < kend; kf += 1.0f) {
-                        const float wxy = fmaxf(1.0f - fabsf(ex), 0.f) * fmaxf(1.0f - fabsf(ey), 0.f);
+                        const float wxy = __saturatef(1.0f - fabsf(ex)) * __saturatef(1.0f - fabsf(ey));
 #pragma unroll
-                        for (int t = 0; t < ZT; ++t) W[t] = fmaf(wxy, fmaxf(1.0f - fabsf(ez - (float)t), 0.f), W[t]);
+                        for (int t = 0; t < ZT; ++t) W[t] = fmaf(wxy, __saturatef(1.0f - fabsf(ez - (float)t)), W[t]);
                         ex += gNx; ey += gNy; ez += gv;
                     }
                 }
@@ -328,9 +331,12 @@ static int launch_gather(cbct_geom *g, AdjGeom &G, const float *sinoI, float *vo
     // rate: 50.5 -> 49.5 ms per 4-channel launch at 256^3 / 400 views).  A preference, set once per instance.
     constexpr int NACC = NM * CB * ZT * NR;
     if constexpr (NACC > 16 && MINB > 0) {
-        static bool carved = false;
-        if (!carved) {
-            carved = true;
+        // the attribute is per device and per function: one bit per device ordinal, set once (thread-safe)
+        static std::atomic<uint64_t> carved{0};
+        int devid = 0;
+        cudaGetDevice(&devid);
+        const uint64_t bit = (uint64_t)1 << (devid & 63);
+        if (!(carved.fetch_or(bit) & bit)) {
             constexpr size_t per_cta = (size_t)NACC * ADJ_BX * ADJ_BY * ADJ_BZ * sizeof(float) + 1024;
             constexpr int pct = (int)((MINB * per_cta * 100 + 228 * 1024 - 1) / (228 * 1024));
             cudaFuncSetAttribute(adjoint_gather_kernel<NR, NM, CB, false, ADJ_BZ, MINB, ZT>,
@@ -349,7 +355,7 @@ static int launch_gather(cbct_geom *g, AdjGeom &G, const float *sinoI, float *vo
         G.split_stride = (size_t)CB * nvox;
         grid.z = nzb * nsplit;
         cbct_prof_begin(g, CBCT_KERNEL_ADJOINT, st);
-        if (G.step < 0.5f) adjoint_gather_kernel<NR, NM, CB, true, ADJ_BZ, MINB, ZT><<<grid, block, 0, st>>>(sinoI, partial, G, vc, 0, 0, sstride, nvox, 0);
+        if (G.fine) adjoint_gather_kernel<NR, NM, CB, true, ADJ_BZ, MINB, ZT><<<grid, block, 0, st>>>(sinoI, partial, G, vc, 0, 0, sstride, nvox, 0);
         else adjoint_gather_kernel<NR, NM, CB, false, ADJ_BZ, MINB, ZT><<<grid, block, 0, st>>>(sinoI, partial, G, vc, 0, 0, sstride, nvox, 0);
         cbct_prof_end(g, CBCT_KERNEL_ADJOINT, st);
         int rc = cbct_check_launch(g, "adjoint_gather_kernel");
@@ -365,7 +371,7 @@ static int launch_gather(cbct_geom *g, AdjGeom &G, const float *sinoI, float *vo
         for (int i = 0; i < n; ++i) vc.cs[i] = make_double2(g->cosphi[q0 + i], g->sinphi[q0 + i]);
         G.nq = n;
         cbct_prof_begin(g, CBCT_KERNEL_ADJOINT, st);
-        if (G.step < 0.5f)
+        if (G.fine)
             adjoint_gather_kernel<NR, NM, CB, true, ADJ_BZ, MINB, ZT><<<grid, block, 0, st>>>(sinoI, vol, G, vc, q0, accumulate_first || q0 > 0,
                                                                             sstride, vstride, vol_z_origin);
         else
@@ -471,6 +477,11 @@ int cbct_launch_adjoint(cbct_geom *g, const float *sino_src, float *vol, int cha
     G.scale = (float)(d.step_vox * d.vox_mm);
     double vmax = fmax(fabs(G.v0), fabs(G.v0 + (d.det_nv - 1) * G.dv));
     G.tz = (float)(vmax / G.sdd);
+    // Window of a (voxel, ray) pair: |mu| <= 1 / |N_d| <= sqrt 2 / H with H = sqrt(sdd^2 + u^2), at L / step samples per
+    // unit mu, i.e. fewer than 2 sqrt 2 (L / H) / step lattice points, L / H = sqrt(1 + v^2 / H^2) <= sqrt(1 + tz^2).
+    // The unrolled loop covers 6; anything that can be longer (steps below 1/2 voxel, or a tall detector: at step 1/2
+    // from |v| / sdd = 0.354, a cone half-angle of 19.5 degrees) takes the variant that walks the rest of the window.
+    G.fine = !(2.0 * M_SQRT2 * sqrt(1.0 + (vmax / G.sdd) * (vmax / G.sdd)) / d.step_vox < 6.0);
     G.nu = d.det_nu; G.nv = d.det_nv; G.nx = d.vol_nx; G.ny = d.vol_ny; G.nz = d.vol_nz;
     const int NR = g->sym_rot;
     const bool mirror = pair || (g->sym_mirror_z && zs0 == 0 && zs1 == d.vol_nz && d.vol_nz > 1);

@@ -28,9 +28,20 @@ static MemKind classify(const void *p)
     }
 }
 
+// Set by begin_call: the caller's stream is being captured into a CUDA graph.  A captured graph bakes in the
+// workspace addresses, and cudaMalloc / cudaFree / cudaDeviceSynchronize are not allowed during capture, so a call
+// that would have to GROW the workspace then fails loudly (CBCT_ERR_UNSUPPORTED) instead: warm the handle up with
+// one uncaptured call of the same shape, or cbct_geom_reserve, first.
+static thread_local bool g_capturing = false;
+
 static int ensure(float **p, size_t *have, size_t need)
 {
     if (*have >= need) return CBCT_OK;
+    if (g_capturing) {
+        cbct_set_cuda_error(cudaErrorStreamCaptureUnsupported, "workspace growth while the stream is capturing "
+                            "(warm up or cbct_geom_reserve first)");
+        return CBCT_ERR_UNSUPPORTED;
+    }
     if (*p) { cudaDeviceSynchronize(); cudaFree(*p); *p = nullptr; *have = 0; }
     cudaError_t e = cudaMalloc((void **)p, need);
     if (e != cudaSuccess) { cbct_set_cuda_error(e, "cudaMalloc(workspace)"); *p = nullptr; return CBCT_ERR_NOMEM; }
@@ -82,6 +93,11 @@ static int begin_call(const cbct_geom *gc, const void *vol, const void *sino, in
     cx.kv = classify(vol);
     cx.ks = classify(sino);
     cx.pageable = (cx.kv == MEM_HOST_PAGEABLE) || (cx.ks == MEM_HOST_PAGEABLE);
+    cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+    if (cudaStreamIsCapturing(cx.st, &cap) != cudaSuccess) { (void)cudaGetLastError(); cap = cudaStreamCaptureStatusNone; }
+    g_capturing = cap != cudaStreamCaptureStatusNone;
+    if (g_capturing && (cx.kv != MEM_DEVICE || cx.ks != MEM_DEVICE)) return CBCT_ERR_UNSUPPORTED;  // host staging uses side streams
+    if (g_capturing && (!cx.g->copy_stream || !cx.g->ev[3])) return CBCT_ERR_UNSUPPORTED;           // never warmed up
     return ensure_streams(cx.g);
 }
 
@@ -448,4 +464,100 @@ extern "C" int cbct_bp_fdk(const cbct_geom *gc, const float *sino, float *vol, i
     if (rc) return rc;
     if (cx.pageable) CBCT_CUDA_TRY(cudaStreamSynchronize(st));
     return CBCT_OK;
+}
+
+// ---------------------------------------------------------------------------
+// Plane ranges of the backprojectors (the unit a multi-GPU caller shards by; also the
+// unit of the streaming path above).  DEVICE pointers.  out[c] holds planes [z0, z1) of channel c; with
+// mirror_pair != 0 (geometry symmetric under z -> -z, z1 <= ceil(nz / 2)) it holds 2 (z1 - z0) - skip planes per
+// channel: [z0, z1) followed by their mirror images [nz - z1 + skip, nz - z0) in ascending order, skip = 1 when
+// the range contains the middle plane of an odd nz (its own image), else 0.  The pair shares every weight.
+// ---------------------------------------------------------------------------
+static int slab_impl(const cbct_geom *gc, const float *sino, float *out, int32_t channels, int32_t z0, int32_t z1,
+                     int32_t mirror_pair, void *stream, int which)
+{
+    CallCtx cx;
+    int rc = begin_call(gc, out, sino, channels, stream, cx);
+    if (rc) return rc;
+    cbct_geom *g = cx.g;
+    cudaStream_t st = cx.st;
+    const int nz = g->d.vol_nz;
+    if (cx.kv != MEM_DEVICE || cx.ks != MEM_DEVICE) return CBCT_ERR_INVALID_ARG;
+    if (z0 < 0 || z1 > nz || z0 >= z1) return CBCT_ERR_INVALID_ARG;
+    if (mirror_pair && (!g->sym_mirror_z || z1 > (nz + 1) / 2)) return CBCT_ERR_INVALID_ARG;
+    const int n = z1 - z0;
+    const int mlo = nz - z1;
+    const int skip = mirror_pair && mlo < z1 ? z1 - mlo : 0;
+    const size_t cstride = cx.plane * (size_t)(mirror_pair ? 2 * n - skip : n);
+    const int morigin = mirror_pair ? mlo + skip - n : CBCT_NO_MIRROR_PAIR;  // plane index stored at out[c] + 0
+    const size_t sino_bytes = cx.nsino * channels * sizeof(float);
+    if (which == 0) {
+        const float *d_sino = sino;
+        if (g->sym_rot > 1) {
+            rc = ensure(&g->ws_sino2, &g->ws_sino2_bytes, sino_bytes);
+            if (rc) return rc;
+            rc = cbct_launch_interleave_views(g, sino, g->ws_sino2, channels, nullptr, st);
+            if (rc) return rc;
+            d_sino = g->ws_sino2;
+        }
+        return cbct_launch_adjoint(g, d_sino, out, channels, z0, z1, cstride, z0, nullptr, 1, st, morigin);
+    }
+    const int pu = cbct_padded_sino_pitch(g), pv = cbct_padded_sino_rows(g);
+    rc = ensure(&g->ws_sino2, &g->ws_sino2_bytes, (size_t)g->d.n_views * pu * pv * channels * sizeof(float));
+    if (rc) return rc;
+    rc = cbct_launch_pad_sino(g, sino, g->ws_sino2, channels, st);
+    if (rc) return rc;
+    return cbct_launch_fdk(g, g->ws_sino2, out, channels, z0, z1, cstride, z0, st, morigin);
+}
+
+extern "C" int cbct_bp_adjoint_slab(const cbct_geom *g, const float *sino, float *out, int32_t channels, int32_t z0,
+                                    int32_t z1, int32_t mirror_pair, void *stream)
+{
+    return slab_impl(g, sino, out, channels, z0, z1, mirror_pair, stream, 0);
+}
+
+extern "C" int cbct_bp_fdk_slab(const cbct_geom *g, const float *sino, float *out, int32_t channels, int32_t z0,
+                                int32_t z1, int32_t mirror_pair, void *stream)
+{
+    return slab_impl(g, sino, out, channels, z0, z1, mirror_pair, stream, 1);
+}
+
+// ---------------------------------------------------------------------------
+// Workspace queries / up-front allocation (so that later calls neither allocate nor synchronise: CUDA graphs)
+// ---------------------------------------------------------------------------
+extern "C" int cbct_geom_workspace_bytes(const cbct_geom *g, uint64_t *out)
+{
+    if (!g || !out) return CBCT_ERR_INVALID_ARG;
+    *out = (uint64_t)g->ws_vol_bytes + g->ws_sino_bytes + g->ws_sino2_bytes + g->ws_stage_bytes + g->ws_blk_in_bytes +
+           g->ws_blk_out_bytes + (g->d_filter_tab ? 3u * (uint64_t)g->d.det_nu * sizeof(float) : 0u);
+    return CBCT_OK;
+}
+
+extern "C" int cbct_geom_reserve(cbct_geom *g, int32_t channels)
+{
+    if (!g || channels < 1) return CBCT_ERR_INVALID_ARG;
+    int rc = have_device();
+    if (rc) return rc;
+    g_capturing = false;
+    rc = ensure_streams(g);
+    if (rc) return rc;
+    const size_t nvol = (size_t)g->d.vol_nx * g->d.vol_ny * g->d.vol_nz;
+    const size_t nsino = (size_t)g->d.n_views * g->d.det_nv * g->d.det_nu;
+    // forward: packed slab buffer(s)
+    const int planes = cbct_plan_slab_planes(g, channels);
+    if (planes < 1) return CBCT_ERR_NOMEM;
+    const int n_slabs = (g->d.vol_nz + planes - 1) / planes;
+    const RayGeom rmax = cbct_make_raygeom(g, 0, planes);
+    size_t vol_bytes = ((size_t)(channels / 4) * (size_t)(rmax.px + CBCT_ROW_SKEW) * rmax.py * rmax.pz +
+                        (size_t)(channels % 4) * cbct_packed_tail_cells(g, rmax)) * (n_slabs > 1 ? 2 : 1) * sizeof(float4);
+    // adjoint on small grids: partial outputs of the view groups
+    const int nsplit = cbct_adjoint_view_splits(g);
+    if (nsplit > 1 && (size_t)nsplit * 8 * nvol * sizeof(float) > vol_bytes) vol_bytes = (size_t)nsplit * 8 * nvol * sizeof(float);
+    rc = ensure(&g->ws_vol, &g->ws_vol_bytes, vol_bytes);
+    if (rc) return rc;
+    // backprojectors: re-laid-out sinogram (view-interleaved / zero-bordered)
+    const size_t psino = (size_t)g->d.n_views * cbct_padded_sino_pitch(g) * cbct_padded_sino_rows(g);
+    rc = ensure(&g->ws_sino2, &g->ws_sino2_bytes, (psino > nsino ? psino : nsino) * channels * sizeof(float));
+    if (rc) return rc;
+    return cbct_ensure_filter_tables(g);
 }

@@ -128,3 +128,125 @@ def test_two_handles_on_two_streams():
     for r, o in zip(ref, outs):
         for a, b in zip(r, o):
             assert torch.equal(a, b)
+
+
+def test_workspace_growth_during_capture_is_refused_and_reserve_avoids_it():
+    """A captured graph bakes in workspace addresses, so a call that would have to GROW the workspace while its
+    stream is capturing must fail loudly (and enqueue nothing) instead of re-allocating; cbct_geom_reserve sizes
+    everything up front, after which more channels than any earlier call capture fine and memory stays flat."""
+    if not torch.cuda.is_available():
+        pytest.fail("gpu-marked tests need a CUDA device (no CPU fallback exists)")
+    from paper_2512_21180_b200 import cbct
+    kw = dict(synth.geom_kwargs(synth.CONFIGS["tiny"]), n_views=6)   # few views: the adjoint needs no partial-sum workspace
+    g = cbct.Geometry(**kw)
+    gen = torch.Generator(device="cuda").manual_seed(7)
+    x = torch.rand((6,) + g.vol_shape, device="cuda", generator=gen)
+    y = torch.empty((6,) + g.sino_shape, device="cuda")
+    x2 = torch.empty_like(x)
+    g.fp(x[:1], y[:1], 1)            # warm-up with ONE channel only
+    g.bp_adjoint(y[:1], x2[:1], 1)
+    torch.cuda.synchronize()
+    side = torch.cuda.Stream()
+    graph = torch.cuda.CUDAGraph()
+    with pytest.raises(cbct.CbctError):
+        with torch.cuda.graph(graph, stream=side):
+            g.fp(x, y, 6)            # needs a larger packed-volume workspace
+    torch.cuda.synchronize()
+    g.reserve(6)
+    before = g.workspace_bytes()
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph, stream=side):
+        g.fp(x, y, 6)
+        g.bp_adjoint(y, x2, 6)
+        g.bp_fdk(y, x2, 6)
+    graph.replay()
+    torch.cuda.synchronize()
+    assert g.workspace_bytes() == before
+    ref = torch.empty_like(y)
+    g.fp(x, ref, 6)
+    torch.cuda.synchronize()
+    assert torch.equal(ref, y)
+
+
+def test_capped_handle_does_not_thrash_its_workspace():
+    """Alternating cbct_fp / cbct_bp_adjoint / cbct_bp_fdk on ONE handle under a work-set cap (host volumes,
+    z-slab streaming): the workspace is shared by forward slabs, output staging and sinogram copies; it may grow
+    during the first round and must stay flat afterwards (no re-allocation per call)."""
+    if not torch.cuda.is_available():
+        pytest.fail("gpu-marked tests need a CUDA device (no CPU fallback exists)")
+    from paper_2512_21180_b200 import cbct
+    kw = dict(synth.geom_kwargs(synth.CONFIGS["tiny"]))
+    kw.update(vol_nz=40, n_views=12, det_off_u_mm=15.0)
+    g = cbct.Geometry(**kw, max_workset_bytes=2500000)
+    C = 3
+    assert g.num_slabs(C) > 2
+    rng = np.random.default_rng(12)
+    vol = torch.from_numpy(rng.random((C,) + g.vol_shape, dtype=np.float32)).pin_memory()
+    sino = torch.from_numpy(rng.random((C,) + g.sino_shape, dtype=np.float32)).cuda()
+    out_s = torch.empty_like(sino)
+    out_v = torch.empty_like(vol).pin_memory()
+    sizes = []
+    for rnd in range(3):
+        g.fp(vol, out_s, C)
+        g.bp_adjoint(sino, out_v, C)
+        g.bp_fdk(sino, out_v, C)
+        g.fp(vol[:2].contiguous().pin_memory(), out_s[:2], 2)      # a smaller call in between
+        torch.cuda.synchronize()
+        sizes.append((g.workspace_bytes(), torch.cuda.memory_allocated()))
+    assert sizes[0][0] > 0
+    assert sizes[1] == sizes[0] and sizes[2] == sizes[0], sizes
+
+
+@pytest.mark.parametrize("over", [dict(n_views=12), dict(n_views=12, vol_nz=27), dict(n_views=7, det_off_v_mm=3.0),
+                                  dict(n_views=10, vol_nx=30, det_off_u_mm=20.0)])
+def test_plane_range_exports_tile_the_whole_volume_calls(oracle_mod, over):
+    """cbct_bp_adjoint_slab / cbct_bp_fdk_slab (the shard of a plane-sharded multi-GPU backprojection): ranges that
+    tile [0, nz), plain and as z-mirror pairs, reassemble the whole-volume result (FDK bit for bit; the adjoint to
+    fp32 summation order) and equal the oracle."""
+    if not torch.cuda.is_available():
+        pytest.fail("gpu-marked tests need a CUDA device (no CPU fallback exists)")
+    from paper_2512_21180_b200 import cbct
+    kw = dict(synth.geom_kwargs(synth.CONFIGS["tiny"]))
+    kw.update(over)
+    g = cbct.Geometry(**kw)
+    og = oracle_mod.Geom(**kw)
+    C = 3
+    nz, ny, nx = g.vol_shape
+    rng = np.random.default_rng(33)
+    sino_h = rng.random((C,) + g.sino_shape, dtype=np.float32)
+    sino = torch.from_numpy(sino_h).cuda()
+    mirror_ok = kw.get("det_off_v_mm", 0.0) == 0.0
+    for whole, slab, ref, tol in ((g.bp_adjoint, g.bp_adjoint_slab, oracle_mod.bp_adjoint(og, sino_h.astype(np.float64)), 1e-4),
+                                  (g.bp_fdk, g.bp_fdk_slab, oracle_mod.bp_fdk(og, sino_h.astype(np.float64)), 1e-5)):
+        full = whole(sino, torch.empty((C,) + g.vol_shape, device="cuda"), C)
+        # plain ranges of ragged sizes
+        got = torch.full_like(full, float("nan"))
+        for z0, z1 in ((0, 5), (5, 6), (6, 19), (19, nz)):
+            buf = torch.full((C, z1 - z0, ny, nx), float("nan"), device="cuda")
+            slab(sino, buf, z0, z1, C)
+            got[:, z0:z1] = buf
+        torch.cuda.synchronize()
+        a, b = got.cpu().numpy().astype(np.float64), full.cpu().numpy().astype(np.float64)
+        assert np.linalg.norm(a - ref) / np.linalg.norm(ref) <= tol
+        assert np.max(np.abs(a - b)) <= 2e-6 * np.max(np.abs(b))
+        if not mirror_ok:
+            with pytest.raises(cbct.CbctError):
+                slab(sino, torch.empty((C, 4, ny, nx), device="cuda"), 0, 2, C, mirror_pair=True)
+            continue
+        # mirror pairs: ranges of the lower half, each with its image
+        nh = (nz + 1) // 2
+        got = torch.full_like(full, float("nan"))
+        for z0, z1 in ((0, 3), (3, 10), (10, nh)):
+            n = g.slab_planes(z0, z1, True)
+            buf = torch.full((C, n, ny, nx), float("nan"), device="cuda")
+            slab(sino, buf, z0, z1, C, mirror_pair=True)
+            k = z1 - z0
+            got[:, z0:z1] = buf[:, :k]
+            got[:, nz - z0 - (n - k):nz - z0] = buf[:, k:]
+        torch.cuda.synchronize()
+        a = got.cpu().numpy().astype(np.float64)
+        assert np.isfinite(a).all()
+        assert np.linalg.norm(a - ref) / np.linalg.norm(ref) <= tol
+        assert np.max(np.abs(a - b)) <= 2e-6 * np.max(np.abs(b))
+        with pytest.raises(cbct.CbctError):
+            slab(sino, torch.empty((C, 2 * nh, ny, nx), device="cuda"), 1, nh + 1, C, mirror_pair=True)

@@ -277,13 +277,37 @@ def test_sampled_variants_match_full(oracle_mod):
     assert np.array_equal(o.bp_fdk_voxels(g, y, vidx), o.bp_fdk(g, y).reshape(2, -1)[:, vidx])
 
 
-def test_tiny_sample_count(oracle_mod):
-    """Tiny config in-support samples: ~68 per ray (32^3 box, 0.5-voxel step)."""
+def _support_box_chords(kw):
+    """Length of every ray inside the open support box -1 < q < N (reading R4), by the slab method on the closed-form
+    rays of tests/analytic.py (PAPER.md:61 geometry) -- no oracle code involved.  Returns chords[V, nv, nu] in mm."""
+    src, d = an.rays(kw)
+    h = kw["vox_mm"]
+    n = np.array([kw["vol_nx"], kw["vol_ny"], kw["vol_nz"]], dtype=np.float64)
+    c = np.array([kw["vol_cx_mm"], kw["vol_cy_mm"], kw["vol_cz_mm"]])
+    lo, hi = c - 0.5 * (n + 1) * h, c + 0.5 * (n + 1) * h      # index -1 and N on each axis
+    with np.errstate(divide="ignore", invalid="ignore"):
+        t0, t1 = (lo - src) / d, (hi - src) / d
+    tmin = np.max(np.minimum(t0, t1), -1)
+    tmax = np.min(np.maximum(t0, t1), -1)
+    return np.clip(tmax - np.maximum(tmin, 0.0), 0.0, None)
+
+
+@pytest.mark.parametrize("name,expected", [("tiny", 5635008), ("small_halffan", 169180088)])
+def test_sample_count_pinned(oracle_mod, name, expected):
+    """The unit of the headline metric (SURVEY.md s.8(d) table: 5.635e6 samples on config 1, 1.692e8 on config 2;
+    the exact integers are the ones the round-1 review obtained from this oracle and matched to that table).
+    Independent of the oracle: a ray holds chord / step lattice points up to +-1, with no bias over many rays, so the
+    total must equal sum(chord) / Delta to a small fraction of a sample per ray.  A closed support 0 <= q <= N-1
+    (64 instead of 67.9 samples per ray on config 1) misses this by 6 %."""
     o = oracle_mod
-    g, _ = G(o)
-    n = o.count_samples(g)
-    rays = 36 * 48 * 48
-    assert 60.0 < n / rays < 75.0
+    kw = synth.geom_kwargs(synth.CONFIGS[name])
+    n = o.count_samples(o.Geom(**kw))
+    assert n == expected
+    chords = _support_box_chords(kw)
+    want = float(np.sum(chords)) / (kw["step_vox"] * kw["vox_mm"])
+    hit = int(np.count_nonzero(chords > 0))
+    assert abs(n - want) <= 0.05 * hit            # |mean phase error| well below 0.05 samples per ray
+    assert abs(n - want) / want < 2e-3
 
 
 def test_p13_redundancy_weight_properties(oracle_mod):
