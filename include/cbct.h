@@ -203,6 +203,11 @@ int cbct_geom_count_samples(const cbct_geom *g, uint64_t *out);
  * (1 = everything resident).  Needs no CUDA device. */
 int cbct_geom_num_slabs(const cbct_geom *g, int32_t channels, int32_t *out);
 
+/* Symmetries of the geometry that the kernels exploit (weights of symmetric voxel / view pairs are equal):
+ * *rotations = 4, 2 or 1 -- views i and i + n_views / rotations see the (centred, for 4: square) grid rotated by
+ * 360 / rotations degrees; *mirror_z = 1 if volume and detector rows are centred in z.  Needs no CUDA device. */
+int cbct_geom_symmetry(const cbct_geom *g, int32_t *rotations, int32_t *mirror_z);
+
 /* Device bytes of workspace the handle owns right now (packed slabs / staging, sinogram copies, tables). */
 int cbct_geom_workspace_bytes(const cbct_geom *g, uint64_t *out);
 

@@ -20,7 +20,7 @@ LIB_PATH = os.path.join(_HERE, "libcbct.so")
 EXPORTS = (
     "cbct_geom_create", "cbct_geom_destroy", "cbct_fp", "cbct_bp_adjoint", "cbct_bp_fdk",
     "cbct_geom_count_samples", "cbct_geom_num_slabs", "cbct_geom_launch_count",
-    "cbct_geom_workspace_bytes", "cbct_geom_reserve", "cbct_bp_adjoint_slab", "cbct_bp_fdk_slab",
+    "cbct_geom_symmetry", "cbct_geom_workspace_bytes", "cbct_geom_reserve", "cbct_bp_adjoint_slab", "cbct_bp_fdk_slab",
     "cbct_geom_profile", "cbct_geom_profile_read",
     "cbct_fdk_filter", "cbct_redundancy_weight", "cbct_geom_redundancy_weights",
     "cbct_fp_residual", "cbct_bp_adjoint_weighted",
@@ -74,6 +74,7 @@ def load_library() -> ctypes.CDLL:
     L.cbct_geom_launch_count.argtypes = [vp, ctypes.POINTER(ctypes.c_uint64)]
     L.cbct_geom_workspace_bytes.argtypes = [vp, ctypes.POINTER(ctypes.c_uint64)]
     L.cbct_geom_reserve.argtypes = [vp, i32]
+    L.cbct_geom_symmetry.argtypes = [vp, ctypes.POINTER(i32), ctypes.POINTER(i32)]
     for name in ("cbct_bp_adjoint_slab", "cbct_bp_fdk_slab"):
         getattr(L, name).argtypes = [vp, vp, vp, i32, i32, i32, i32, vp]
     L.cbct_geom_profile.argtypes = [vp, ctypes.c_int]
@@ -306,6 +307,12 @@ class Geometry:
         out = ctypes.c_int32()
         _check(load_library().cbct_geom_num_slabs(self._h, channels, ctypes.byref(out)))
         return int(out.value)
+
+    def symmetry(self):
+        """cbct_geom_symmetry: (rotations in {4, 2, 1}, z-mirror flag) of the geometry."""
+        r, m = ctypes.c_int32(), ctypes.c_int32()
+        _check(load_library().cbct_geom_symmetry(self._h, ctypes.byref(r), ctypes.byref(m)))
+        return int(r.value), bool(m.value)
 
     def workspace_bytes(self) -> int:
         """cbct_geom_workspace_bytes: device bytes of workspace the handle owns right now."""

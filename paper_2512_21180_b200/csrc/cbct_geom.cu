@@ -281,6 +281,14 @@ extern "C" int cbct_geom_profile_read(cbct_geom *g, int kernel, double *ms_total
     return CBCT_OK;
 }
 
+extern "C" int cbct_geom_symmetry(const cbct_geom *g, int32_t *rotations, int32_t *mirror_z)
+{
+    if (!g || !rotations || !mirror_z) return CBCT_ERR_INVALID_ARG;
+    *rotations = g->sym_rot;
+    *mirror_z = g->sym_mirror_z ? 1 : 0;
+    return CBCT_OK;
+}
+
 extern "C" int cbct_geom_launch_count(const cbct_geom *g, uint64_t *out)
 {
     if (!g || !out) return CBCT_ERR_INVALID_ARG;

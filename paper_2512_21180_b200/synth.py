@@ -37,14 +37,42 @@ CONFIGS = {
     "large_512": _cfg("large_512", 512, 1.0, 512, 0.8, 720, 115.0, 4, 1005, 300, True),
 }
 
+# Variants of config 4 / config 3 whose view angles are what a real scanner delivers (432-944
+# projections per scan "to approximate actual variability ... in real data"; gantry angle read-outs are not
+# equispaced): `angle_jitter_deg` = half-width of a seeded uniform jitter added to the equispaced angles (sorted),
+# and a view count that is no multiple of 4.  Neither has the quarter-turn symmetry between views.
+CONFIGS["multichannel_256_jitter"] = dict(CONFIGS["multichannel_256"], name="multichannel_256_jitter",
+                                          angle_jitter_deg=0.2)
+CONFIGS["pyramid_256_jitter"] = dict(CONFIGS["pyramid_256"], name="pyramid_256_jitter", angle_jitter_deg=0.2)
+CONFIGS["multichannel_256_v402"] = dict(CONFIGS["multichannel_256"], name="multichannel_256_v402", n_views=402)
+CONFIGS["pyramid_256_v402"] = dict(CONFIGS["pyramid_256"], name="pyramid_256_v402", n_views=402)
+
+
+def view_angles(cfg: dict):
+    """Per-view angles in radians, or None for the equispaced default 2 pi i / n.  Jittered lists are seeded
+    (default_rng(seed + 7)), uniform in +-angle_jitter_deg about the equispaced angles, sorted."""
+    jit = float(cfg.get("angle_jitter_deg", 0.0))
+    if jit == 0.0:
+        return None
+    n = cfg["n_views"]
+    rng = np.random.default_rng(cfg["seed"] + 7)
+    a = 2.0 * np.pi * np.arange(n) / n + np.deg2rad(rng.uniform(-jit, jit, size=n))
+    return [float(x) for x in np.sort(a)]
+
+
 GEOM_KEYS = ("sid_mm", "sdd_mm", "n_views", "det_nu", "det_nv", "det_du_mm", "det_dv_mm",
              "det_off_u_mm", "det_off_v_mm", "vol_nx", "vol_ny", "vol_nz", "vox_mm",
              "vol_cx_mm", "vol_cy_mm", "vol_cz_mm", "step_vox")
 
 
 def geom_kwargs(cfg: dict) -> dict:
-    """The plain geometry numbers of a config (keys shared by both descriptors)."""
-    return {k: cfg[k] for k in GEOM_KEYS}
+    """The plain geometry numbers of a config (keys shared by both descriptors), plus `angles_rad` when the
+    config's view angles are not the equispaced default."""
+    kw = {k: cfg[k] for k in GEOM_KEYS}
+    ang = view_angles(cfg)
+    if ang is not None:
+        kw["angles_rad"] = ang
+    return kw
 
 
 def _quat_to_rot(q):
@@ -99,7 +127,7 @@ def rasterise(ellipsoids, n: int, vox_mm: float, cylinder: bool = False,
 def config_ellipsoids(cfg: dict):
     n, h = cfg["vol_nx"], cfg["vox_mm"]
     name = cfg["name"]
-    if name.startswith("pyramid") or name == "multichannel_256":
+    if name.startswith("pyramid") or name.startswith("multichannel_256"):
         # one phantom defined once in mm on the finest (256^3 / 2 mm) grid
         return draw_ellipsoids(cfg["seed"], cfg["n_ellipsoids"], 512.0, 2.0)
     return draw_ellipsoids(cfg["seed"], cfg["n_ellipsoids"], n * h, h)
