@@ -31,28 +31,11 @@
 // NM = 2 voxels mirrored in z (ray iv <-> nv-1-iv).  One weight evaluation
 // then feeds NR * NM * CB accumulators.
 #include <atomic>
+#include <cstdlib>
 
 #include "cbct_device.cuh"
+#include "cbct_adjoint.cuh"
 
-struct AdjGeom {
-    double sid, sdd, inv_sdd;
-    double u0, du, inv_du, v0, dv, inv_dv;  // detector coordinate of pixel 0, pitch (voxel units)
-    double x0, y0, z0;                      // world coordinate (voxel units) of voxel index 0
-    double inv_step;
-    float step, scale;                      // ray step (voxel units); Delta in mm
-    float tz;                               // max |v| / sdd over the detector
-    int fine;                               // the sample window of a (voxel, ray) pair can hold more than 6 lattice points
-    int nu, nv, nx, ny, nz;
-    int bx, by;                             // base domain: ix < bx, iy < by
-    int bz0, bz1;                           // base planes [bz0, bz1)
-    int mz_origin;                          // first stored plane of the z-mirrored voxels' output (NM = 2)
-    int nq;                                 // views in this launch
-    int nbase;                              // n_views / NR: views i and i + nbase differ by 360/NR degrees
-    // small grids do not fill the GPU with one thread per base voxel: the views of a launch are then split
-    // over `nsplit` groups of CTAs, each writing its partial sums to its own copy of the output
-    int nsplit, views_per_split;
-    size_t split_stride;                    // floats between the partial outputs of consecutive splits
-};
 
 // out[c][iq][iv][iu][p] = in[c][iq + p nq][iv][iu], iq < nq = n_views / NR
 // (the NR views related by a grid rotation side by side, one vector load)
@@ -82,8 +65,6 @@ interleave_views_kernel(const float *__restrict__ in, float *__restrict__ out, i
 
 // A warp covers 8 (x) x 4 (y) voxels of one plane: compact on the detector, so the lanes walk similar
 // (iu, iv) ranges (measured 32.0 -> 29.5 ms per channel against 32 x 1; 4 x 8 and 8 x 2 x 2: 29.8, 29.7).
-#define ADJ_BX 8
-#define ADJ_BY 16
 
 // ADJ_BZ threads along z per CTA; MINB = CTAs per SM the register allocation aims for (0: the compiler's choice);
 // ZT = consecutive planes per thread.  Voxels (x, y, z + t) see the same e_x, e_y on a ray and e_z shifted by
@@ -100,7 +81,10 @@ adjoint_gather_kernel(const float *__restrict__ sinoI, float *__restrict__ vol, 
     const int iy = blockIdx.y * ADJ_BY + threadIdx.y;
     const int nzb = (G.bz1 - G.bz0 + ADJ_BZ * ZT - 1) / (ADJ_BZ * ZT);
     const int split = blockIdx.z / nzb;
-    const int iz = G.bz0 + ((blockIdx.z - split * nzb) * ADJ_BZ + threadIdx.z) * ZT;  // first of the ZT planes
+    // plane blocks are launched from the top of the range downwards: with the z-mirror the base planes are the
+    // lower half, whose top planes lie in the cone for every view (the heaviest CTAs): started last, they would
+    // leave most SMs idle at the end of the launch
+    const int iz = G.bz0 + ((nzb - 1 - (blockIdx.z - split * nzb)) * ADJ_BZ + threadIdx.z) * ZT;  // first of the ZT planes
     const bool valid = ix < G.bx && iy < G.by && iz < G.bz1;
     vol += split * G.split_stride;
     const int q_begin = split * G.views_per_split, q_end = min(G.nq, q_begin + G.views_per_split);
@@ -315,6 +299,15 @@ reduce_splits_kernel(const float *__restrict__ partial, float *__restrict__ out,
     }
 }
 
+int cbct_launch_reduce_splits(cbct_geom *g, const float *partial, float *out, size_t nvox, int cb, int nsplit,
+                              size_t out_cstride, cudaStream_t st)
+{
+    size_t blocks = (nvox * cb + 255) / 256;
+    if (blocks > 148u * 16u) blocks = 148u * 16u;
+    reduce_splits_kernel<<<(unsigned)blocks, 256, 0, st>>>(partial, out, nvox, cb, nsplit, out_cstride);
+    return cbct_check_launch(g, "reduce_splits_kernel");
+}
+
 template <int NR, int NM, int CB, int ADJ_BZ = 1, int MINB = 0, int ZT = 1>
 static int launch_gather(cbct_geom *g, AdjGeom &G, const float *sinoI, float *vol, int accumulate_first,
                          size_t sstride, size_t vstride, int vol_z_origin, float *partial, int nsplit, cudaStream_t st)
@@ -360,10 +353,7 @@ static int launch_gather(cbct_geom *g, AdjGeom &G, const float *sinoI, float *vo
         cbct_prof_end(g, CBCT_KERNEL_ADJOINT, st);
         int rc = cbct_check_launch(g, "adjoint_gather_kernel");
         if (rc) return rc;
-        size_t blocks = (nvox * CB + 255) / 256;
-        if (blocks > 148u * 16u) blocks = 148u * 16u;
-        reduce_splits_kernel<<<(unsigned)blocks, 256, 0, st>>>(partial, vol, nvox, CB, nsplit, vstride);
-        return cbct_check_launch(g, "reduce_splits_kernel");
+        return cbct_launch_reduce_splits(g, partial, vol, nvox, CB, nsplit, vstride, st);
     }
     for (int q0 = 0; q0 < nq_total; q0 += CBCT_VIEWS_PER_LAUNCH) {
         int n = nq_total - q0;
@@ -390,10 +380,24 @@ static int launch_gather_channels(cbct_geom *g, AdjGeom &G, const float *sinoI, 
                                   cudaStream_t st)
 {
     int c = 0;
+    static const int column_mode = [] { const char *e = getenv("CBCT_ADJ_COLUMN"); return e ? atoi(e) : 1; }();
+    // the partial-output workspace is sized for the regime of the grid (cbct_adjoint_partial_floats): 8 channels of
+    // the voxel kernel on small grids, 2 channels of the column kernel on large ones
+    const bool small = cbct_adjoint_small_grid(g) && nsplit > 1;
+    float *const partial_voxel = small ? partial : nullptr;
+    const int nsplit_voxel = small ? nsplit : 1;
     while (c < channels) {
         int left = channels - c, rc;
         const float *s = sinoI + c * sstride;
         float *v = vol + c * vstride;
+        // column-walk kernel (cbct_adjoint_column.cu): blocks of 1 or 2 channels on grids large enough to fill the
+        // GPU with one thread per column chunk (small grids keep the view-split path of the voxel kernel)
+        if (column_mode && !small && (left < 4 || column_mode >= 2)) {
+            const int cb = left >= 2 ? 2 : 1;
+            rc = cbct_launch_adjoint_column(g, G, NR, NM, cb, s, v, sstride, vstride, vol_z_origin, partial, nsplit, st);
+            if (rc == CBCT_OK) { c += cb; continue; }
+            if (rc != 1) return rc;
+        }
         // One weight evaluation feeds NR * NM * CB accumulators: 16 in registers; geometries with fewer
         // symmetries (irregular view angles, off-centre grids) make it up with more channels per thread.
         // 32 accumulators per weight evaluation when the channels are there; the sums over views then live in
@@ -401,33 +405,33 @@ static int launch_gather_channels(cbct_geom *g, AdjGeom &G, const float *sinoI, 
         // 8 channels: 17.5 -> 12.8 ms per channel; with 128-thread CTAs the 20 resident warps drift apart by
         // several views and evict each other's pixels from L1: hit rate 56 %, no gain)
         if constexpr (NR * NM == 8) {
-            if (left >= 4) { rc = launch_gather<NR, NM, 4, 2, 2>(g, G, s, v, 0, sstride, vstride, vol_z_origin, partial, nsplit, st); c += 4; if (rc) return rc; continue; }
+            if (left >= 4) { rc = launch_gather<NR, NM, 4, 2, 2>(g, G, s, v, 0, sstride, vstride, vol_z_origin, partial_voxel, nsplit_voxel, st); c += 4; if (rc) return rc; continue; }
         }
         if constexpr (NR * NM == 4) {
-            if (left >= 8) { rc = launch_gather<NR, NM, 8, 2, 2>(g, G, s, v, 0, sstride, vstride, vol_z_origin, partial, nsplit, st); c += 8; if (rc) return rc; continue; }
+            if (left >= 8) { rc = launch_gather<NR, NM, 8, 2, 2>(g, G, s, v, 0, sstride, vstride, vol_z_origin, partial_voxel, nsplit_voxel, st); c += 8; if (rc) return rc; continue; }
         }
         if constexpr (NR * NM <= 2) {
             // 16 accumulators in registers; the 256-thread CTA pays with two symmetric voxels (24.0 -> 22.0 ms
             // per channel with irregular view angles), not with one (31.0 -> 34.6)
-            if (NR * NM == 2 && left >= 8) { rc = launch_gather<NR, NM, 8, 2, 2>(g, G, s, v, 0, sstride, vstride, vol_z_origin, partial, nsplit, st); c += 8; if (rc) return rc; continue; }
-            if (left >= 8) { rc = launch_gather<NR, NM, 8>(g, G, s, v, 0, sstride, vstride, vol_z_origin, partial, nsplit, st); c += 8; if (rc) return rc; continue; }
+            if (NR * NM == 2 && left >= 8) { rc = launch_gather<NR, NM, 8, 2, 2>(g, G, s, v, 0, sstride, vstride, vol_z_origin, partial_voxel, nsplit_voxel, st); c += 8; if (rc) return rc; continue; }
+            if (left >= 8) { rc = launch_gather<NR, NM, 8>(g, G, s, v, 0, sstride, vstride, vol_z_origin, partial_voxel, nsplit_voxel, st); c += 8; if (rc) return rc; continue; }
         }
         if constexpr (NR * NM <= 4) {
-            if (left >= 4) { rc = launch_gather<NR, NM, 4>(g, G, s, v, 0, sstride, vstride, vol_z_origin, partial, nsplit, st); c += 4; if (rc) return rc; continue; }
+            if (left >= 4) { rc = launch_gather<NR, NM, 4>(g, G, s, v, 0, sstride, vstride, vol_z_origin, partial_voxel, nsplit_voxel, st); c += 4; if (rc) return rc; continue; }
         }
         // fewer than 4 channels at full symmetry: two planes per thread share the horizontal tap weights, the
         // per-pixel set-up and the pixel loads (256^3 / 400 views: 28.5 -> 26.9 ms at 1 channel, 35.0 -> 31.4 ms at
         // 2); it does not pay on small grids (128^3 and below), where the longer pixel loops cost more
         if constexpr (NR * NM == 8) {
             if ((size_t)G.nx * G.ny * G.nz >= ((size_t)1 << 23)) {
-                if (left >= 2) { rc = launch_gather<NR, NM, 2, 1, 0, 2>(g, G, s, v, 0, sstride, vstride, vol_z_origin, partial, nsplit, st); c += 2; }
-                else { rc = launch_gather<NR, NM, 1, 1, 0, 2>(g, G, s, v, 0, sstride, vstride, vol_z_origin, partial, nsplit, st); c += 1; }
+                if (left >= 2) { rc = launch_gather<NR, NM, 2, 1, 0, 2>(g, G, s, v, 0, sstride, vstride, vol_z_origin, partial_voxel, nsplit_voxel, st); c += 2; }
+                else { rc = launch_gather<NR, NM, 1, 1, 0, 2>(g, G, s, v, 0, sstride, vstride, vol_z_origin, partial_voxel, nsplit_voxel, st); c += 1; }
                 if (rc) return rc;
                 continue;
             }
         }
-        if (left >= 2) { rc = launch_gather<NR, NM, 2>(g, G, s, v, 0, sstride, vstride, vol_z_origin, partial, nsplit, st); c += 2; }
-        else { rc = launch_gather<NR, NM, 1>(g, G, s, v, 0, sstride, vstride, vol_z_origin, partial, nsplit, st); c += 1; }
+        if (left >= 2) { rc = launch_gather<NR, NM, 2>(g, G, s, v, 0, sstride, vstride, vol_z_origin, partial_voxel, nsplit_voxel, st); c += 2; }
+        else { rc = launch_gather<NR, NM, 1>(g, G, s, v, 0, sstride, vstride, vol_z_origin, partial_voxel, nsplit_voxel, st); c += 1; }
         if (rc) return rc;
     }
     return CBCT_OK;
@@ -439,16 +443,37 @@ static int launch_gather_channels(cbct_geom *g, AdjGeom &G, const float *sinoI, 
 // is used only when the launch covers the whole grid.
 // Number of view groups the adjoint uses for this geometry (1 = no splitting): enough to give the GPU
 // about a million threads when one thread per base voxel would not.
+static size_t adjoint_base_threads(const cbct_geom *g)
+{
+    const cbct_geom_desc &d = g->d;
+    size_t threads = (size_t)d.vol_nx * d.vol_ny * d.vol_nz / ((size_t)g->sym_rot * (g->sym_mirror_z ? 2 : 1));
+    return threads ? threads : 1;
+}
+
+bool cbct_adjoint_small_grid(const cbct_geom *g) { return adjoint_base_threads(g) < 2000000; }
+
 int cbct_adjoint_view_splits(const cbct_geom *g)
 {
     const cbct_geom_desc &d = g->d;
     if (d.n_views > CBCT_VIEWS_PER_LAUNCH) return 1;
-    size_t threads = (size_t)d.vol_nx * d.vol_ny * d.vol_nz / ((size_t)g->sym_rot * (g->sym_mirror_z ? 2 : 1));
-    if (threads == 0) threads = 1;
-    size_t s = (2000000 + threads - 1) / threads;
+    if (!cbct_adjoint_small_grid(g)) {
+        // large grids (column kernel): 4 view groups per tile even out the load of the SMs; not under a work-set
+        // cap (the partial outputs are whole volumes) and not for a handful of views
+        return (d.max_workset_bytes == 0 && d.n_views >= 64) ? 4 : 1;
+    }
+    size_t s = (2000000 + adjoint_base_threads(g) - 1) / adjoint_base_threads(g);
     if (s > 32) s = 32;
     if (s > (size_t)d.n_views / 8) s = (size_t)d.n_views / 8;
     return s < 1 ? 1 : (int)s;
+}
+
+// floats of workspace the partial outputs of `cbct_adjoint_view_splits(g)` view groups need
+size_t cbct_adjoint_partial_floats(const cbct_geom *g)
+{
+    const int nsplit = cbct_adjoint_view_splits(g);
+    if (nsplit <= 1) return 0;
+    const size_t nvol = (size_t)g->d.vol_nx * g->d.vol_ny * g->d.vol_nz;
+    return (size_t)nsplit * (cbct_adjoint_small_grid(g) ? 8 : 2) * nvol;
 }
 
 // `partial` (nsplit > 1 only): workspace of nsplit * 8 * nx * ny * nz floats; used when the launch covers the

@@ -401,11 +401,11 @@ static int adjoint_impl(const cbct_geom *gc, const float *sino, float *vol, int3
         if (rc) return rc;
         d_sino = g->ws_sino2;
     }
-    // small grids: split the views over groups of CTAs (partial outputs in workspace, then reduced)
+    // the views of a launch split over groups of CTAs (partial outputs in workspace, then reduced)
     int nsplit = cx.kv == MEM_DEVICE ? cbct_adjoint_view_splits(g) : 1;
     float *partial = nullptr;
     if (nsplit > 1) {
-        rc = ensure(&g->ws_vol, &g->ws_vol_bytes, (size_t)nsplit * 8 * cx.nvol * sizeof(float));
+        rc = ensure(&g->ws_vol, &g->ws_vol_bytes, cbct_adjoint_partial_floats(g) * sizeof(float));
         if (rc) return rc;
         partial = g->ws_vol;
     }
@@ -541,7 +541,6 @@ extern "C" int cbct_geom_reserve(cbct_geom *g, int32_t channels)
     g_capturing = false;
     rc = ensure_streams(g);
     if (rc) return rc;
-    const size_t nvol = (size_t)g->d.vol_nx * g->d.vol_ny * g->d.vol_nz;
     const size_t nsino = (size_t)g->d.n_views * g->d.det_nv * g->d.det_nu;
     // forward: packed slab buffer(s)
     const int planes = cbct_plan_slab_planes(g, channels);
@@ -551,8 +550,7 @@ extern "C" int cbct_geom_reserve(cbct_geom *g, int32_t channels)
     size_t vol_bytes = ((size_t)(channels / 4) * (size_t)(rmax.px + CBCT_ROW_SKEW) * rmax.py * rmax.pz +
                         (size_t)(channels % 4) * cbct_packed_tail_cells(g, rmax)) * (n_slabs > 1 ? 2 : 1) * sizeof(float4);
     // adjoint on small grids: partial outputs of the view groups
-    const int nsplit = cbct_adjoint_view_splits(g);
-    if (nsplit > 1 && (size_t)nsplit * 8 * nvol * sizeof(float) > vol_bytes) vol_bytes = (size_t)nsplit * 8 * nvol * sizeof(float);
+    if (cbct_adjoint_partial_floats(g) * sizeof(float) > vol_bytes) vol_bytes = cbct_adjoint_partial_floats(g) * sizeof(float);
     rc = ensure(&g->ws_vol, &g->ws_vol_bytes, vol_bytes);
     if (rc) return rc;
     // backprojectors: re-laid-out sinogram (view-interleaved / zero-bordered)

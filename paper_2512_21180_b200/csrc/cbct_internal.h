@@ -124,7 +124,9 @@ int cbct_launch_redundancy_weight(cbct_geom *g, const float *in, float *out, int
 int cbct_launch_adjoint(cbct_geom *g, const float *sino_src, float *vol, int channels, int zs0, int zs1,
                         size_t vol_channel_stride, int vol_z_origin, float *partial, int nsplit, cudaStream_t st,
                         int mirror_z_origin = CBCT_NO_MIRROR_PAIR);
-int cbct_adjoint_view_splits(const cbct_geom *g);  // view groups for small grids (1 = none)
+int cbct_adjoint_view_splits(const cbct_geom *g);   // view groups per tile of the adjoint (1 = none)
+bool cbct_adjoint_small_grid(const cbct_geom *g);    // fewer than 2 million base voxels: the voxel kernel splits views
+size_t cbct_adjoint_partial_floats(const cbct_geom *g);  // workspace floats of the view groups' partial outputs
 int cbct_launch_pad_sino(cbct_geom *g, const float *src, float *dst, int channels, cudaStream_t st);
 // FDK backprojection from the padded sinogram into vol planes [zs0, zs1)
 int cbct_launch_fdk(cbct_geom *g, const float *padded_sino, float *vol, int channels, int zs0, int zs1,
