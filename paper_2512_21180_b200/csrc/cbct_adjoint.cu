@@ -31,7 +31,6 @@
 // NM = 2 voxels mirrored in z (ray iv <-> nv-1-iv).  One weight evaluation
 // then feeds NR * NM * CB accumulators.
 #include <atomic>
-#include <cstdlib>
 
 #include "cbct_device.cuh"
 #include "cbct_adjoint.cuh"
@@ -380,7 +379,6 @@ static int launch_gather_channels(cbct_geom *g, AdjGeom &G, const float *sinoI, 
                                   cudaStream_t st)
 {
     int c = 0;
-    static const int column_mode = [] { const char *e = getenv("CBCT_ADJ_COLUMN"); return e ? atoi(e) : 1; }();
     // the partial-output workspace is sized for the regime of the grid (cbct_adjoint_partial_floats): 8 channels of
     // the voxel kernel on small grids, 2 channels of the column kernel on large ones
     const bool small = cbct_adjoint_small_grid(g) && nsplit > 1;
@@ -392,7 +390,8 @@ static int launch_gather_channels(cbct_geom *g, AdjGeom &G, const float *sinoI, 
         float *v = vol + c * vstride;
         // column-walk kernel (cbct_adjoint_column.cu): blocks of 1 or 2 channels on grids large enough to fill the
         // GPU with one thread per column chunk (small grids keep the view-split path of the voxel kernel)
-        if (column_mode && !small && (left < 4 || column_mode >= 2)) {
+        // (with 4 or more channels the voxel kernel's 32 accumulators per weight win: 12.2 against 13.0 ms per channel)
+        if (!small && left < 4) {
             const int cb = left >= 2 ? 2 : 1;
             rc = cbct_launch_adjoint_column(g, G, NR, NM, cb, s, v, sstride, vstride, vol_z_origin, partial, nsplit, st);
             if (rc == CBCT_OK) { c += cb; continue; }
@@ -457,9 +456,10 @@ int cbct_adjoint_view_splits(const cbct_geom *g)
     const cbct_geom_desc &d = g->d;
     if (d.n_views > CBCT_VIEWS_PER_LAUNCH) return 1;
     if (!cbct_adjoint_small_grid(g)) {
-        // large grids (column kernel): 4 view groups per tile even out the load of the SMs; not under a work-set
+        // large grids (column kernel): 8 view groups per tile even out the load of the SMs; not under a work-set
         // cap (the partial outputs are whole volumes) and not for a handful of views
-        return (d.max_workset_bytes == 0 && d.n_views >= 64) ? 4 : 1;
+        if (d.max_workset_bytes != 0 || d.n_views < 64) return 1;
+        return d.n_views >= 128 ? 8 : 4;   // measured at 256^3 / 400 views, 1 channel: 21.1 (none), 18.6, 16.7, 16.0 ms
     }
     size_t s = (2000000 + adjoint_base_threads(g) - 1) / adjoint_base_threads(g);
     if (s > 32) s = 32;
