@@ -443,8 +443,7 @@ extern "C" int cbct_bp_fdk(const cbct_geom *gc, const float *sino, float *vol, i
                             [&](const float *ds, float *dv, int, int nc) { return cbct_bp_fdk(gc, ds, dv, nc, stream); });
 
     // zero-bordered, rotation-interleaved copy of the sinogram (cbct_fdk.cu)
-    const int pu = cbct_padded_sino_pitch(g), pv = cbct_padded_sino_rows(g);
-    const size_t psino = (size_t)g->d.n_views * pu * pv * channels;
+    const size_t psino = cbct_padded_sino_floats(g) * channels;
     const size_t sino_bytes = cx.nsino * channels * sizeof(float);
     const float *d_sino = sino;
     if (cx.ks != MEM_DEVICE) {
@@ -502,8 +501,7 @@ static int slab_impl(const cbct_geom *gc, const float *sino, float *out, int32_t
         }
         return cbct_launch_adjoint(g, d_sino, out, channels, z0, z1, cstride, z0, nullptr, 1, st, morigin);
     }
-    const int pu = cbct_padded_sino_pitch(g), pv = cbct_padded_sino_rows(g);
-    rc = ensure(&g->ws_sino2, &g->ws_sino2_bytes, (size_t)g->d.n_views * pu * pv * channels * sizeof(float));
+    rc = ensure(&g->ws_sino2, &g->ws_sino2_bytes, cbct_padded_sino_floats(g) * channels * sizeof(float));
     if (rc) return rc;
     rc = cbct_launch_pad_sino(g, sino, g->ws_sino2, channels, st);
     if (rc) return rc;
@@ -554,7 +552,7 @@ extern "C" int cbct_geom_reserve(cbct_geom *g, int32_t channels)
     rc = ensure(&g->ws_vol, &g->ws_vol_bytes, vol_bytes);
     if (rc) return rc;
     // backprojectors: re-laid-out sinogram (view-interleaved / zero-bordered)
-    const size_t psino = (size_t)g->d.n_views * cbct_padded_sino_pitch(g) * cbct_padded_sino_rows(g);
+    const size_t psino = cbct_padded_sino_floats(g);
     rc = ensure(&g->ws_sino2, &g->ws_sino2_bytes, (psino > nsino ? psino : nsino) * channels * sizeof(float));
     if (rc) return rc;
     return cbct_ensure_filter_tables(g);

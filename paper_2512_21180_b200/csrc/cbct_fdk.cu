@@ -23,7 +23,17 @@ int cbct_check_launch(cbct_geom *g, const char *what)
     return CBCT_OK;
 }
 
-// out[c][ib][pv][pu][p] = in[c][ib + p nb][v][u] inside the detector, 0 on the border
+// Re-layout of the sinogram for the backprojection kernel: one RECORD per padded pixel (pv, pu) of base view ib, zero
+// outside the detector (boundary rule R10 without bounds tests), so that one vector load serves
+//   NR = 4 (16 B): the pixel in the 4 views ib + p nb related by quarter turns   (4 LDG.128 = 4 taps of 4 voxels)
+//   NR = 2 ( 8 B): the pixel in the 2 views ib, ib + nb                          (4 LDG.64  = 4 taps of 2 voxels)
+//   NR = 1 (16 B): the 2 x 2 taps (v, u), (v, u + 1), (v + 1, u), (v + 1, u + 1)  (1 LDG.128 = 4 taps of 1 voxel)
+// i.e. 16 B through L1 per voxel-view whatever the symmetry of the view angles (scalar taps made geometries without
+// rotation symmetry twice as slow: 8.6 against 4.6 ms per channel at 256^3 / 400 views; the quad records: 6.7 ms --
+// they cost L1 capacity, every pixel being stored four times; for NR = 2 the same trick -- records (u, u + 1) x
+// 2 views, 2 LDG.128 -- measured slower than the plain pair of views, 6.7 against 5.8 ms, and was dropped).
+#define FDK_RECF(NR) ((NR) == 2 ? 2 : 4)   // floats per record
+
 template <int NR>
 __global__ void __launch_bounds__(256)
 pad_sino_kernel(const float *__restrict__ in, float *__restrict__ out, int nu, int nv, int pu, int pv, int nb,
@@ -37,17 +47,13 @@ pad_sino_kernel(const float *__restrict__ in, float *__restrict__ out, int nu, i
         const int v = (int)(t % pv) - CBCT_PAD;
         t /= pv;
         const size_t ib = t % nb, c = t / nb;
-        float vals[NR];
-#pragma unroll
-        for (int r = 0; r < NR; ++r) vals[r] = 0.f;
-        if (u >= 0 && u < nu && v >= 0 && v < nv) {
-            const float *src = in + (c * NR * nb + ib) * img + (size_t)v * nu + u;
-#pragma unroll
-            for (int r = 0; r < NR; ++r) vals[r] = __ldg(src + (size_t)r * nb * img);
-        }
-        if (NR == 4) reinterpret_cast<float4 *>(out)[e] = make_float4(vals[0], vals[1], vals[2], vals[NR - 1]);
-        else if (NR == 2) reinterpret_cast<float2 *>(out)[e] = make_float2(vals[0], vals[NR - 1]);
-        else out[e] = vals[0];
+        const float *src = in + (c * NR * nb + ib) * img;
+        auto px = [&](int r, int vv, int uu) -> float {
+            return (uu >= 0 && uu < nu && vv >= 0 && vv < nv) ? __ldg(src + (size_t)r * nb * img + (size_t)vv * nu + uu) : 0.f;
+        };
+        if (NR == 4) reinterpret_cast<float4 *>(out)[e] = make_float4(px(0, v, u), px(1, v, u), px(2, v, u), px(NR - 1, v, u));
+        else if (NR == 2) reinterpret_cast<float2 *>(out)[e] = make_float2(px(0, v, u), px(NR - 1, v, u));
+        else reinterpret_cast<float4 *>(out)[e] = make_float4(px(0, v, u), px(0, v, u + 1), px(0, v + 1, u), px(0, v + 1, u + 1));
     }
 }
 
@@ -71,26 +77,53 @@ struct FdkViews {
 // an integer cell and an fp32 fraction, so the fp32 work along z only ever
 // sees small magnitudes (|t| < ~32): coordinate error ~1e-6 px instead of the
 // 1.5e-5 px ulp of a raw fp32 coordinate near 256 (DESIGN.md s.6).
-template <int NR, int NM, int ZB>
+// CB channels per thread share the whole per-(x, y, view) set-up (the fp64 coordinates, the weight) and the
+// per-voxel row arithmetic; their records lie `sino_cstride` float4 apart.
+template <int NR, int NM, int ZB, int CB>
 __global__ void __launch_bounds__(FDK_BX *FDK_BY)
 fdk_kernel(const float *__restrict__ sinoP, float *__restrict__ vol, const __grid_constant__ FdkGeom G,
-           const __grid_constant__ FdkViews V, int q0, int accumulate, int vol_z_origin)
+           const __grid_constant__ FdkViews V, int q0, int accumulate, int vol_z_origin, size_t sino_cstride,
+           size_t vol_cstride)
 {
     const int ix = blockIdx.x * FDK_BX + threadIdx.x;
     const int iy = blockIdx.y * FDK_BY + threadIdx.y;
     const int izb = G.bz0 + blockIdx.z * ZB;
     if (ix >= G.bx || iy >= G.by) return;
     const double X = G.x0 + (double)ix, Y = G.y0 + (double)iy, Z0 = G.z0 + (double)izb;
-    float acc[NM][ZB][NR];
+    float acc[CB][NM][ZB][NR];
 #pragma unroll
-    for (int m = 0; m < NM; ++m)
+    for (int c = 0; c < CB; ++c)
 #pragma unroll
-        for (int k = 0; k < ZB; ++k)
+        for (int m = 0; m < NM; ++m)
 #pragma unroll
-            for (int r = 0; r < NR; ++r) acc[m][k][r] = 0.f;
+            for (int k = 0; k < ZB; ++k)
+#pragma unroll
+                for (int r = 0; r < NR; ++r) acc[c][m][k][r] = 0.f;
     const size_t pimg = (size_t)G.pu * G.pv;
-    const int rowstride = G.pu * NR;
     int a_prev = q0 / G.nbase;
+
+    // bilinear interpolation of the NR views from the records of rows `row`, `row + 1` at column ju (rec points at
+    // the record (row, ju)): fraction au along u, fv along v; adds w * value into dst[0 .. NR)
+    constexpr int RECF = FDK_RECF(NR);
+    const int rowstride = G.pu * RECF;
+    auto taps = [&](const float *__restrict__ rec, float au, float fv, float w, float (&dst)[NR]) {
+        if (NR == 1) {
+            const float4 t = __ldg(reinterpret_cast<const float4 *>(rec));   // (v u, v u+1, v+1 u, v+1 u+1)
+            const float b0 = fmaf(au, t.y - t.x, t.x), b1 = fmaf(au, t.w - t.z, t.z);
+            dst[0] = fmaf(w, fmaf(fv, b1 - b0, b0), dst[0]);
+        } else {
+            float y00[NR], y01[NR], y10[NR], y11[NR];
+            load_views<NR>(rec, y00);
+            load_views<NR>(rec + NR, y01);
+            load_views<NR>(rec + rowstride, y10);
+            load_views<NR>(rec + rowstride + NR, y11);
+#pragma unroll
+            for (int rr = 0; rr < NR; ++rr) {
+                const float b0 = fmaf(au, y01[rr] - y00[rr], y00[rr]), b1 = fmaf(au, y11[rr] - y10[rr], y10[rr]);
+                dst[rr] = fmaf(w, fmaf(fv, b1 - b0, b0), dst[rr]);
+            }
+        }
+    };
 
     for (int q = 0; q < G.n_views; ++q) {
         // during the views of block a the accumulator of the r-th rotated voxel is
@@ -98,9 +131,11 @@ fdk_kernel(const float *__restrict__ sinoP, float *__restrict__ vol, const __gri
         const int a = (q0 + q) / G.nbase, ib = (q0 + q) - a * G.nbase;
         if (NR > 1 && a != a_prev) {
 #pragma unroll
-            for (int m = 0; m < NM; ++m)
+            for (int c = 0; c < CB; ++c)
 #pragma unroll
-                for (int k = 0; k < ZB; ++k) rotate_views<NR>(acc[m][k], NR - (a - a_prev));
+                for (int m = 0; m < NM; ++m)
+#pragma unroll
+                    for (int k = 0; k < ZB; ++k) rotate_views<NR>(acc[c][m][k], NR - (a - a_prev));
             a_prev = a;
         }
         const double c = V.cs[q].x, s = V.cs[q].y;
@@ -121,7 +156,7 @@ fdk_kernel(const float *__restrict__ sinoP, float *__restrict__ vol, const __gri
         const int jv0 = (int)base;
         const float f0 = (float)(fv0 - base), dfv = (float)dfv_d;
         const float lo = 1.0f - (float)jv0, hi = (float)(G.fv_max - base);
-        const float *p = sinoP + ((size_t)ib * pimg + ju) * NR;
+        const float *p = sinoP + ((size_t)ib * pimg + ju) * RECF;
 #pragma unroll
         for (int k = 0; k < ZB; ++k) {
             const float t = fminf(fmaxf(fmaf((float)k, dfv, f0), lo), hi);
@@ -129,31 +164,11 @@ fdk_kernel(const float *__restrict__ sinoP, float *__restrict__ vol, const __gri
             float av;
             cbct_cell_frac(t - 0.5f, jr, av);
             const int row = jv0 + jr;
-            {
-                const float *q00 = p + row * rowstride;
-                float y00[NR], y01[NR], y10[NR], y11[NR];
-                load_views<NR>(q00, y00);
-                load_views<NR>(q00 + NR, y01);
-                load_views<NR>(q00 + rowstride, y10);
-                load_views<NR>(q00 + rowstride + NR, y11);
 #pragma unroll
-                for (int rr = 0; rr < NR; ++rr) {
-                    const float b0 = fmaf(au, y01[rr] - y00[rr], y00[rr]), b1 = fmaf(au, y11[rr] - y10[rr], y10[rr]);
-                    acc[0][k][rr] = fmaf(w, fmaf(av, b1 - b0, b0), acc[0][k][rr]);
-                }
-            }
-            if (NM == 2) {  // voxel mirrored in z: rows pv-2-row and pv-1-row, fraction 1 - av
-                const float *q00 = p + (G.pv - 2 - row) * rowstride;
-                float y00[NR], y01[NR], y10[NR], y11[NR];
-                load_views<NR>(q00, y00);
-                load_views<NR>(q00 + NR, y01);
-                load_views<NR>(q00 + rowstride, y10);
-                load_views<NR>(q00 + rowstride + NR, y11);
-#pragma unroll
-                for (int rr = 0; rr < NR; ++rr) {
-                    const float b0 = fmaf(au, y01[rr] - y00[rr], y00[rr]), b1 = fmaf(au, y11[rr] - y10[rr], y10[rr]);
-                    acc[NM - 1][k][rr] = fmaf(w, fmaf(av, b0 - b1, b1), acc[NM - 1][k][rr]);
-                }
+            for (int cc = 0; cc < CB; ++cc) {
+                taps(p + cc * sino_cstride + row * rowstride, au, av, w, acc[cc][0][k]);
+                // voxel mirrored in z: rows pv-2-row and pv-1-row, fraction 1 - av
+                if (NM == 2) taps(p + cc * sino_cstride + (G.pv - 2 - row) * rowstride, au, 1.0f - av, w, acc[cc][NM - 1][k]);
             }
         }
     }
@@ -167,7 +182,8 @@ fdk_kernel(const float *__restrict__ sinoP, float *__restrict__ vol, const __gri
             if (izk >= G.bz1) continue;
             const int z = m == 0 ? izk : G.nz - 1 - izk;
             if (m == 1 && z == izk) continue;  // middle plane of an odd nz is its own mirror image
-            rotate_views<NR>(acc[m][k], a_prev);
+#pragma unroll
+            for (int cc = 0; cc < CB; ++cc) rotate_views<NR>(acc[cc][m][k], a_prev);
 #pragma unroll
             for (int r = 0; r < NR; ++r) {
                 int x = ix, y = iy;
@@ -179,7 +195,11 @@ fdk_kernel(const float *__restrict__ sinoP, float *__restrict__ vol, const __gri
                     x = G.nx - 1 - ix; y = G.ny - 1 - iy;
                 }
                 float *dst = vol + ((size_t)(z - (m == 0 ? vol_z_origin : G.mz_origin)) * G.ny + y) * G.nx + x;
-                *dst = accumulate ? *dst + acc[m][k][r] : acc[m][k][r];
+#pragma unroll
+                for (int cc = 0; cc < CB; ++cc) {
+                    float *d = dst + cc * vol_cstride;
+                    *d = accumulate ? *d + acc[cc][m][k][r] : acc[cc][m][k][r];
+                }
             }
         }
 }
@@ -187,6 +207,12 @@ fdk_kernel(const float *__restrict__ sinoP, float *__restrict__ vol, const __gri
 // ---------------------------------------------------------------------------
 // launchers
 // ---------------------------------------------------------------------------
+// floats per channel of the re-laid-out sinogram: one 16-byte record per padded pixel of every base view
+size_t cbct_padded_sino_floats(const cbct_geom *g)
+{
+    return (size_t)(g->d.n_views / g->sym_rot) * cbct_padded_sino_pitch(g) * cbct_padded_sino_rows(g) * FDK_RECF(g->sym_rot);
+}
+
 int cbct_launch_pad_sino(cbct_geom *g, const float *src, float *dst, int channels, cudaStream_t st)
 {
     const int NR = g->sym_rot, nb = g->d.n_views / NR;
@@ -200,12 +226,21 @@ int cbct_launch_pad_sino(cbct_geom *g, const float *src, float *dst, int channel
     return cbct_check_launch(g, "pad_sino_kernel");
 }
 
+// Two channels per thread share the fp64 set-up of a (column, view) pair.  It pays only without rotation symmetry
+// (8 channels with jittered angles: 6.0 against 6.7 ms per channel); with NR = 4 the 125 registers of the
+// two-channel instance cut the resident warps from 24 to 16 per SM and the kernel, which waits on its loads, slows
+// from 4.7 to 5.3 ms per channel.
+#ifndef FDK_CB
+#define FDK_CB 2
+#endif
+
 template <int NR, int NM, int ZB>
 static int launch_fdk(cbct_geom *g, FdkGeom &G, const float *padded, float *vol, int channels, size_t vstride,
                       int vol_z_origin, cudaStream_t st)
 {
     const cbct_geom_desc &d = g->d;
-    const size_t sstride = (size_t)d.n_views * G.pu * G.pv;  // floats per channel of the re-laid-out sinogram
+    const size_t sstride = cbct_padded_sino_floats(g);  // floats per channel of the re-laid-out sinogram
+    const float *rec = padded;
     G.nbase = d.n_views / NR;
     FdkViews fv;
     dim3 block(FDK_BX, FDK_BY);
@@ -215,10 +250,18 @@ static int launch_fdk(cbct_geom *g, FdkGeom &G, const float *padded, float *vol,
         if (n > CBCT_VIEWS_PER_LAUNCH) n = CBCT_VIEWS_PER_LAUNCH;
         for (int i = 0; i < n; ++i) fv.cs[i] = make_double2(g->cosphi[q0 + i], g->sinphi[q0 + i]);
         G.n_views = n;
-        for (int c = 0; c < channels; ++c) {
+        int c = 0;
+        while (c < channels) {
             cbct_prof_begin(g, CBCT_KERNEL_FDK, st);
-            fdk_kernel<NR, NM, ZB><<<grid, block, 0, st>>>(padded + c * sstride, vol + c * vstride, G, fv, q0, q0 > 0,
-                                                           vol_z_origin);
+            if (FDK_CB >= 2 && NR == 1 && channels - c >= 2) {
+                fdk_kernel<NR, NM, ZB, 2><<<grid, block, 0, st>>>(rec + c * sstride, vol + c * vstride, G, fv, q0, q0 > 0,
+                                                                  vol_z_origin, sstride, vstride);
+                c += 2;
+            } else {
+                fdk_kernel<NR, NM, ZB, 1><<<grid, block, 0, st>>>(rec + c * sstride, vol + c * vstride, G, fv, q0, q0 > 0,
+                                                                  vol_z_origin, sstride, vstride);
+                c += 1;
+            }
             cbct_prof_end(g, CBCT_KERNEL_FDK, st);
             int rc = cbct_check_launch(g, "fdk_kernel");
             if (rc) return rc;

@@ -99,6 +99,7 @@ size_t cbct_packed_volume_cells(const RayGeom &r);  // float4 cells per channel 
 size_t cbct_packed_tail_cells(const cbct_geom *g, const RayGeom &r);  // ... per channel left over by the groups of 4
 int cbct_padded_sino_pitch(const cbct_geom *g);
 int cbct_padded_sino_rows(const cbct_geom *g);
+size_t cbct_padded_sino_floats(const cbct_geom *g);  // per channel of the FDK kernel's record layout (cbct_fdk.cu)
 int cbct_plan_slab_planes(const cbct_geom *g, int channels);  // planes per z-slab, <1 = cap too small
 
 // --- kernel launchers; all enqueue on `st` ----------------------------------
