@@ -39,9 +39,11 @@ class LireOperators:
     """Geometry handles and work buffers of the three scales (full grid n^3, detector n x n, n_views views)."""
 
     def __init__(self, n: int = 256, n_views: int = 400, latent_channels: int = 8, device="cuda",
-                 fov_mm: float = FOV_MM, panel_mm: float = PANEL_MM, offset_mm: float = OFFSET_MM):
-        if n % 4 or n_views % 4:
-            raise cbct.CbctError("n and n_views must be divisible by 4 (three scales)")
+                 fov_mm: float = FOV_MM, panel_mm: float = PANEL_MM, offset_mm: float = OFFSET_MM, angles_rad=None):
+        """Any view count (the scanner delivers 432-944 projections) and, with `angles_rad`, any angle
+        list: scale 1/f keeps views 0, f, 2f, ... of the full list (reading R14), ceil(n_views / f) of them."""
+        if n % 4:
+            raise cbct.CbctError("n must be divisible by 4 (three scales of average pooling)")
         self.n, self.n_views, self.C = n, n_views, latent_channels
         self.half = latent_channels // 2
         self.dev = torch.device(device)
@@ -49,16 +51,21 @@ class LireOperators:
         for f in SCALES:
             m = n // f
             self.geoms[f] = cbct.Geometry(
-                **self.geom_kwargs(n, n_views, f, fov_mm, panel_mm, offset_mm))
+                **self.geom_kwargs(n, n_views, f, fov_mm, panel_mm, offset_mm, angles_rad))
         g = self.geoms[1]
         self.V = g.fov(torch.empty(g.vol_shape, device=self.dev))   # PAPER.md:169, once per geometry
 
     @staticmethod
-    def geom_kwargs(n, n_views, f, fov_mm=FOV_MM, panel_mm=PANEL_MM, offset_mm=OFFSET_MM) -> dict:
+    def geom_kwargs(n, n_views, f, fov_mm=FOV_MM, panel_mm=PANEL_MM, offset_mm=OFFSET_MM, angles_rad=None) -> dict:
         """Geometry of the scale alpha = 1 / f (plain numbers; the tests hand the same ones to the oracle)."""
+        import math
         m = n // f
-        return dict(n_views=n_views // f, det_nu=m, det_nv=m, det_du_mm=panel_mm / m, det_dv_mm=panel_mm / m,
-                    det_off_u_mm=offset_mm, vol_nx=m, vol_ny=m, vol_nz=m, vox_mm=fov_mm / m)
+        kw = dict(n_views=-(-n_views // f), det_nu=m, det_nv=m, det_du_mm=panel_mm / m, det_dv_mm=panel_mm / m,
+                  det_off_u_mm=offset_mm, vol_nx=m, vol_ny=m, vol_nz=m, vox_mm=fov_mm / m)
+        if angles_rad is not None or n_views % f:
+            full = list(angles_rad) if angles_rad is not None else [2.0 * math.pi * i / n_views for i in range(n_views)]
+            kw["angles_rad"] = full[::f]
+        return kw
 
     def _new(self, *shape):
         return torch.empty(shape, device=self.dev, dtype=torch.float32)
@@ -134,7 +141,10 @@ class LireOperators:
                     m2 = 2 * m
                     f = cbct.upsample(f.contiguous(), self._new(C, m2, m2, m2), 2)
                     nxt = self.geoms[SCALES[i + 1]]
-                    hdual = cbct.upsample(hdual.contiguous(), self._new(C, *nxt.sino_shape), 2)
+                    nv_c, nv_f = g.sino_shape[0], nxt.sino_shape[0]
+                    hdual = cbct.upsample(hdual.contiguous(), self._new(C, 2 * nv_c, *nxt.sino_shape[1:]), 2)
+                    if nv_f != 2 * nv_c:      # view counts that are no multiple of 4: fine view k <- coarse view k // 2
+                        hdual = hdual[:, :nv_f].contiguous()
         return outputs
 
 

@@ -11,11 +11,11 @@ pytestmark = pytest.mark.gpu
 
 torch = pytest.importorskip("torch")
 
-N, VIEWS, C = 32, 16, 8
+N, C = 32, 8
 GEO = dict(fov_mm=256.0, panel_mm=240.0, offset_mm=40.0)
 
 
-def oracle_sequence(o, y_raw):
+def oracle_sequence(o, y_raw, VIEWS):
     """Alg. 1 with the oracle's operators; mirrors lire_ops.LireOperators.reconstruct_operators line by line."""
     from paper_2512_21180_b200.lire_ops import SCALES, LireOperators
     h = C // 2
@@ -53,11 +53,12 @@ def oracle_sequence(o, y_raw):
         outs.append(x)
         hd, f = np.roll(hd, 1, axis=0), np.roll(f, 1, axis=0)
         if i < len(SCALES) - 1:
-            f, hd = o.upsample(f, 2), o.upsample(hd, 2)
+            f, hd = o.upsample(f, 2), o.upsample(hd, 2)[:, :G[SCALES[i + 1]].n_views]
     return outs
 
 
-def test_lire_operator_sequence_matches_oracle(oracle_mod):
+@pytest.mark.parametrize("VIEWS", [16, 18, 21])
+def test_lire_operator_sequence_matches_oracle(oracle_mod, VIEWS):
     if not torch.cuda.is_available():
         pytest.fail("gpu-marked tests need a CUDA device (no CPU fallback exists)")
     from paper_2512_21180_b200 import lire_ops
@@ -67,7 +68,7 @@ def test_lire_operator_sequence_matches_oracle(oracle_mod):
     timings = {}
     got = ops.reconstruct_operators(torch.from_numpy(y_raw).cuda(), timings)
     torch.cuda.synchronize()
-    ref = oracle_sequence(oracle_mod, y_raw.astype(np.float64))
+    ref = oracle_sequence(oracle_mod, y_raw.astype(np.float64), VIEWS)
     assert len(got) == len(ref) == 3
     for k, (a, r) in enumerate(zip(got, ref)):
         a = a.cpu().numpy().astype(np.float64)
