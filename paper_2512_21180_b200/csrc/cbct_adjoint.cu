@@ -164,6 +164,16 @@ adjoint_gather_kernel(const float *__restrict__ sinoI, float *__restrict__ vol, 
                 // a_v - t in place of a_v
                 const float zb = fmaf(fabsf(v), zcull, 1.0f);
                 if (ZT == 1 ? fabsf(av) >= zb : (av <= -zb || av >= (float)(ZT - 1) + zb)) continue;
+                // 4 channels (the 32-accumulator instance): channel 0's pixels are requested before the weight arithmetic,
+                // which covers their latency, and each further channel's while the one before is used (software
+                // pipeline; the compiler otherwise places every load right before its first use, where 36 % of the
+                // stall samples sat): 49.5 -> 47.7 ms per launch.  With 8 channels it gains nothing.
+                constexpr bool PIPE = CB == 4;
+                float yc0[PIPE ? NR : 1], yc1[PIPE ? NR : 1];
+                if (PIPE) {
+                    load_views<NR>(sq + i0, reinterpret_cast<float (&)[NR]>(yc0));
+                    if (NM == 2) load_views<NR>(sq + i1, reinterpret_cast<float (&)[NR]>(yc1));
+                }
                 const float L = L2 * invL;
                 const float invg = L * inv_stepf;  // samples per unit lambda
                 const float g = G.step * invL;     // lambda per sample
@@ -204,6 +214,27 @@ adjoint_gather_kernel(const float *__restrict__ sinoI, float *__restrict__ vol, 
 #pragma unroll
                 for (int t = 0; t < ZT; ++t) any = any || W[t] != 0.f;
                 if (!any) continue;
+                if constexpr (PIPE) {
+#pragma unroll
+                    for (int cc = 0; cc < CB; ++cc) {
+                        float yn0[NR], yn1[NR];
+                        if (cc + 1 < CB) {   // next channel's pixels in flight while this one's are used
+                            load_views<NR>(sq + (cc + 1) * sino_cstride + i0, yn0);
+                            if (NM == 2) load_views<NR>(sq + (cc + 1) * sino_cstride + i1, yn1);
+                        }
+#pragma unroll
+                        for (int t = 0; t < ZT; ++t)
+#pragma unroll
+                            for (int r = 0; r < NR; ++r) {
+                                accv[cc * ZT + t][r] = fmaf(W[t], yc0[PIPE ? r : 0], accv[cc * ZT + t][r]);
+                                if (NM == 2) accv[(NM - 1) * CB * ZT + cc * ZT + t][r] = fmaf(W[t], yc1[PIPE ? r : 0], accv[(NM - 1) * CB * ZT + cc * ZT + t][r]);
+                            }
+                        if (cc + 1 < CB) {
+#pragma unroll
+                            for (int r = 0; r < NR; ++r) { yc0[PIPE ? r : 0] = yn0[r]; if (NM == 2) yc1[PIPE ? r : 0] = yn1[r]; }
+                        }
+                    }
+                } else {
 #pragma unroll
                 for (int cc = 0; cc < CB; ++cc) {
                     float y[NR];
@@ -220,6 +251,7 @@ adjoint_gather_kernel(const float *__restrict__ sinoI, float *__restrict__ vol, 
                             for (int r = 0; r < NR; ++r)
                                 accv[(NM - 1) * CB * ZT + cc * ZT + t][r] = fmaf(W[t], y[r], accv[(NM - 1) * CB * ZT + cc * ZT + t][r]);
                     }
+                }
                 }
             }
         }
@@ -454,7 +486,7 @@ bool cbct_adjoint_small_grid(const cbct_geom *g) { return adjoint_base_threads(g
 int cbct_adjoint_view_splits(const cbct_geom *g)
 {
     const cbct_geom_desc &d = g->d;
-    if (d.n_views > CBCT_VIEWS_PER_LAUNCH) return 1;
+    if (d.n_views > CBCT_VIEWS_PER_LAUNCH && cbct_adjoint_small_grid(g)) return 1;
     if (!cbct_adjoint_small_grid(g)) {
         // large grids (column kernel): 8 view groups per tile even out the load of the SMs; not under a work-set
         // cap (the partial outputs are whole volumes) and not for a handful of views

@@ -283,20 +283,25 @@ static int launch_column(cbct_geom *g, AdjGeom &G, const float *sinoI, float *vo
     dim3 block(ADJ_BX, ADJC_BY, 1);
     const int nch = (G.bz1 - G.bz0 + ZC - 1) / ZC;
     dim3 grid((G.bx + ADJ_BX - 1) / ADJ_BX, (G.by + ADJC_BY - 1) / ADJC_BY, nch);
-    if (partial && nsplit > 1 && nq_total <= CBCT_VIEWS_PER_LAUNCH) {
-        // one launch, the views split over nsplit CTAs per tile into partial outputs of the whole grid, then reduced
+    if (partial && nsplit > 1) {
+        // the views of every launch (chunks of 512) split over nsplit CTAs per tile into partial outputs of the whole
+        // grid -- group s of every chunk adds into partial volume s -- then reduced in a fixed order
         const size_t nvox = (size_t)G.nx * G.ny * G.nz;
-        for (int i = 0; i < nq_total; ++i) vc.cs[i] = make_double2(g->cosphi[i], g->sinphi[i]);
-        G.nq = nq_total;
         G.nsplit = nsplit;
-        G.views_per_split = (nq_total + nsplit - 1) / nsplit;
         G.split_stride = (size_t)CB * nvox;
         grid.z = nch * nsplit;
-        cbct_prof_begin(g, CBCT_KERNEL_ADJOINT, st);
-        kernel<<<grid, block, smem, st>>>(sinoI, partial, G, vc, 0, 0, sstride, nvox, 0);
-        cbct_prof_end(g, CBCT_KERNEL_ADJOINT, st);
-        int rc = cbct_check_launch(g, "adjoint_column_kernel");
-        if (rc) return rc;
+        for (int q0 = 0; q0 < nq_total; q0 += CBCT_VIEWS_PER_LAUNCH) {
+            int n = nq_total - q0;
+            if (n > CBCT_VIEWS_PER_LAUNCH) n = CBCT_VIEWS_PER_LAUNCH;
+            for (int i = 0; i < n; ++i) vc.cs[i] = make_double2(g->cosphi[q0 + i], g->sinphi[q0 + i]);
+            G.nq = n;
+            G.views_per_split = (n + nsplit - 1) / nsplit;
+            cbct_prof_begin(g, CBCT_KERNEL_ADJOINT, st);
+            kernel<<<grid, block, smem, st>>>(sinoI, partial, G, vc, q0, q0 > 0, sstride, nvox, 0);
+            cbct_prof_end(g, CBCT_KERNEL_ADJOINT, st);
+            int rc = cbct_check_launch(g, "adjoint_column_kernel");
+            if (rc) return rc;
+        }
         return cbct_launch_reduce_splits(g, partial, vol, nvox, CB, nsplit, vstride, st);
     }
     G.nsplit = 1; G.views_per_split = CBCT_VIEWS_PER_LAUNCH; G.split_stride = 0;
