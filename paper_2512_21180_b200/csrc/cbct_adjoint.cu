@@ -423,8 +423,13 @@ static int launch_gather_channels(cbct_geom *g, AdjGeom &G, const float *sinoI, 
         // column-walk kernel (cbct_adjoint_column.cu): blocks of 1 or 2 channels on grids large enough to fill the
         // GPU with one thread per column chunk (small grids keep the view-split path of the voxel kernel)
         // (with 4 or more channels the voxel kernel's 32 accumulators per weight win: 12.2 against 13.0 ms per channel)
-        if (!small && left < 4) {
-            const int cb = left >= 2 ? 2 : 1;
+        // Without rotation symmetry (NR * NM <= 2: irregular angle lists) the column kernel also takes the wide
+        // blocks, 8 / (NR * NM) channels per thread: its window then holds the same 8 accumulators per plane as the
+        // single-channel instance of a fully symmetric geometry.
+        if (!small && (left < 4 || NR * NM <= 2)) {
+            int cb = left >= 2 ? 2 : 1;
+            if (NR * NM <= 2 && left >= 4) cb = 4;
+            if (NR * NM == 1 && left >= 8) cb = 8;
             rc = cbct_launch_adjoint_column(g, G, NR, NM, cb, s, v, sstride, vstride, vol_z_origin, partial, nsplit, st);
             if (rc == CBCT_OK) { c += cb; continue; }
             if (rc != 1) return rc;
@@ -505,7 +510,7 @@ size_t cbct_adjoint_partial_floats(const cbct_geom *g)
     const int nsplit = cbct_adjoint_view_splits(g);
     if (nsplit <= 1) return 0;
     const size_t nvol = (size_t)g->d.vol_nx * g->d.vol_ny * g->d.vol_nz;
-    return (size_t)nsplit * (cbct_adjoint_small_grid(g) ? 8 : 2) * nvol;
+    return (cbct_adjoint_small_grid(g) ? (size_t)nsplit * 8 : (size_t)16) * nvol;   // large grids: nsplit * CB <= 16
 }
 
 // `partial` (nsplit > 1 only): workspace of nsplit * 8 * nx * ny * nz floats; used when the launch covers the

@@ -323,8 +323,17 @@ template <int NR, int NM>
 static int launch_column_cb(cbct_geom *g, AdjGeom &G, int CB, const float *sinoI, float *vol, size_t sstride,
                             size_t vstride, int vol_z_origin, float *partial, int nsplit, cudaStream_t st)
 {
+    // the partial outputs of the view groups take nsplit * CB volumes: at most 16 (cbct_adjoint_partial_floats)
+    if (nsplit * CB > 16) nsplit = 16 / CB;
     if (CB == 1) return launch_column<NR, NM, 1>(g, G, sinoI, vol, sstride, vstride, vol_z_origin, partial, nsplit, st);
     if (CB == 2) return launch_column<NR, NM, 2>(g, G, sinoI, vol, sstride, vstride, vol_z_origin, partial, nsplit, st);
+    // geometries with few symmetric images fill the window's 8 accumulators per plane with channels instead
+    if constexpr (NR * NM <= 2) {
+        if (CB == 4) return launch_column<NR, NM, 4>(g, G, sinoI, vol, sstride, vstride, vol_z_origin, partial, nsplit, st);
+    }
+    if constexpr (NR * NM == 1) {
+        if (CB == 8) return launch_column<NR, NM, 8>(g, G, sinoI, vol, sstride, vstride, vol_z_origin, partial, nsplit, st);
+    }
     return 1;
 }
 

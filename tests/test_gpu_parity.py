@@ -246,6 +246,9 @@ _HALFFAN_128 = dict(det_nu=128, det_nv=128, det_du_mm=3.2, det_dv_mm=3.2, det_of
     (dict(_HALFFAN_128, vol_nx=256, vol_ny=256, vol_nz=128, vox_mm=2.0, n_views=66), 2),                  # NR 2, NM 2
     (dict(_HALFFAN_128, vol_nx=160, vol_ny=160, vol_nz=161, vox_mm=3.0, n_views=64, irregular=True), 1),  # NR 1, NM 2, odd nz
     (dict(_HALFFAN_128, vol_nx=128, vol_ny=128, vol_nz=128, vox_mm=4.0, n_views=130, vol_cz_mm=6.0, vol_cx_mm=-4.0), 2),  # none
+    (dict(_HALFFAN_128, vol_nx=160, vol_ny=160, vol_nz=160, vox_mm=3.0, n_views=64, irregular=True), 5),  # NR 1, NM 2: blocks of 4 + 1
+    (dict(_HALFFAN_128, vol_nx=128, vol_ny=128, vol_nz=128, vox_mm=4.0, n_views=64, vol_cz_mm=6.0, irregular=True), 9),  # none: 8 + 1
+    (dict(_HALFFAN_128, vol_nx=128, vol_ny=128, vol_nz=128, vox_mm=4.0, n_views=64, det_off_v_mm=4.0, irregular=True), 6),  # none: 4 + 2
     (dict(det_nu=48, det_nv=48, det_du_mm=8.0, det_dv_mm=8.0, det_off_u_mm=100.0, vol_nx=256, vol_ny=256, vol_nz=256,
           vox_mm=2.0, n_views=1040), 1),   # more views than one launch chunk: the groups accumulate over the chunks
 ])
