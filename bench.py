@@ -441,12 +441,17 @@ def main():
     names = {"fp": ("fp4_pair_kernel" if (C % 4 == 0 or quarter_turns)
                     else ("fp_kernel" if C < 4 else "fp4_pair_kernel+fp_kernel")),
              "adjoint": None, "fdk": "fdk_kernel"}
-    # adjoint: blocks of 4 (or 8) channels take the voxel kernel; the remaining 1-3 channels take the column-walk
-    # kernel on grids of 2 million base voxels or more (cbct_adjoint.cu: launch_gather_channels)
-    large = g.n_vol // (rotations * (2 if mirror else 1)) >= 2000000
-    tail = C % 4 if rotations * (2 if mirror else 1) == 8 else (C % 8) % 4
-    names["adjoint"] = ("adjoint_gather_kernel" if not (large and tail) else
-                        ("adjoint_column_kernel" if C < 4 else "adjoint_gather_kernel+adjoint_column_kernel"))
+    # adjoint (cbct_adjoint.cu: launch_gather_channels), on grids of 2 million base voxels or more: with rotation
+    # symmetry, blocks of 4 (or 8) channels take the voxel kernel and the remaining 1-3 channels the column-walk kernel;
+    # without it (irregular angle lists) the column-walk kernel takes every block
+    images = rotations * (2 if mirror else 1)
+    large = g.n_vol // images >= 2000000
+    tail = C % 4 if images == 8 else (C % 8) % 4
+    if large and images <= 2:
+        names["adjoint"] = "adjoint_column_kernel"
+    else:
+        names["adjoint"] = ("adjoint_gather_kernel" if not (large and tail) else
+                            ("adjoint_column_kernel" if C < 4 else "adjoint_gather_kernel+adjoint_column_kernel"))
     l1_peak = 148 * L1_BYTES_PER_CLK_SM * sm_hz / 1e9
     issue_peak = 148 * ISSUE_LANES_PER_CLK_SM * sm_hz / 1e9
     models = work_models(C, n_samples, n_vv, rotations, mirror)

@@ -408,7 +408,7 @@ static int launch_gather(cbct_geom *g, AdjGeom &G, const float *sinoI, float *vo
 template <int NR, int NM>
 static int launch_gather_channels(cbct_geom *g, AdjGeom &G, const float *sinoI, float *vol, int channels,
                                   size_t sstride, size_t vstride, int vol_z_origin, float *partial, int nsplit,
-                                  cudaStream_t st)
+                                  cudaStream_t st, const float *sino_ci, int ci_groups)
 {
     int c = 0;
     // the partial-output workspace is sized for the regime of the grid (cbct_adjoint_partial_floats): 8 channels of
@@ -430,7 +430,11 @@ static int launch_gather_channels(cbct_geom *g, AdjGeom &G, const float *sinoI, 
             int cb = left >= 2 ? 2 : 1;
             if (NR * NM <= 2 && left >= 4) cb = 4;
             if (NR * NM == 1 && left >= 8) cb = 8;
-            rc = cbct_launch_adjoint_column(g, G, NR, NM, cb, s, v, sstride, vstride, vol_z_origin, partial, nsplit, st);
+            // NR = 1: the caller may have interleaved the channels in groups of 4 (one LDG.128 per pixel and group
+            // instead of 4 scalar loads); groups cover channels [0, 4 ci_groups)
+            int ci = 1;
+            if (NR == 1 && cb >= 4 && sino_ci && c % 4 == 0 && c + cb <= 4 * ci_groups) { ci = 4; s = sino_ci + c * sstride; }
+            rc = cbct_launch_adjoint_column(g, G, NR, NM, cb, ci, s, v, sstride, vstride, vol_z_origin, partial, nsplit, st);
             if (rc == CBCT_OK) { c += cb; continue; }
             if (rc != 1) return rc;
         }
@@ -504,6 +508,39 @@ int cbct_adjoint_view_splits(const cbct_geom *g)
     return s < 1 ? 1 : (int)s;
 }
 
+// The column kernel's preconditions (cbct_adjoint_column.cu) from the geometry alone: the 6-sample window and the
+// three-plane identity hold on every detector row.
+static bool column_kernel_serves(const cbct_geom *g)
+{
+    const cbct_geom_desc &d = g->d;
+    const double v0 = -0.5 * (d.det_nv - 1) * d.det_dv_mm + d.det_off_v_mm;
+    const double tz = fmax(fabs(v0), fabs(v0 + (d.det_nv - 1) * d.det_dv_mm)) / d.sdd_mm;
+    return 2.0 * M_SQRT2 * sqrt(1.0 + tz * tz) / d.step_vox < 6.0 && (float)tz < 0.35f;
+}
+
+// Channels of a call that the adjoint wants interleaved in groups of 4 (NR = 1 geometries on grids the column
+// kernel serves): 4 * (channels / 4), or 0.
+int cbct_adjoint_channel_groups(const cbct_geom *g, int channels, bool device_volume)
+{
+    if (g->sym_rot != 1 || channels < 4 || !column_kernel_serves(g)) return 0;
+    if (cbct_adjoint_small_grid(g) && device_volume && cbct_adjoint_view_splits(g) > 1) return 0;  // voxel kernel's view groups
+    return channels / 4;
+}
+
+// out[gq][view][pix][k] = in[4 gq + k][view][pix]: the rotation-interleaving kernel with "views per rotation block"
+// = all views and "channels" = groups (weights != nullptr: times w(u), the fused P*(w y))
+int cbct_launch_interleave_channels(cbct_geom *g, const float *sino, float *out, int groups, const float *weights,
+                                    cudaStream_t st)
+{
+    const int nq = g->d.n_views;
+    const size_t img = (size_t)g->d.det_nv * g->d.det_nu;
+    const size_t n = (size_t)groups * nq * img;
+    size_t blocks = (n + 255) / 256;
+    if (blocks > 148u * 16u) blocks = 148u * 16u;
+    interleave_views_kernel<4><<<(unsigned)blocks, 256, 0, st>>>(sino, out, nq, img, groups, weights, g->d.det_nu);
+    return cbct_check_launch(g, "interleave_views_kernel");
+}
+
 // floats of workspace the partial outputs of `cbct_adjoint_view_splits(g)` view groups need
 size_t cbct_adjoint_partial_floats(const cbct_geom *g)
 {
@@ -520,7 +557,7 @@ size_t cbct_adjoint_partial_floats(const cbct_geom *g)
 // plane index mirror_z_origin of the same buffer.
 int cbct_launch_adjoint(cbct_geom *g, const float *sino_src, float *vol, int channels, int zs0, int zs1,
                         size_t vol_channel_stride, int vol_z_origin, float *partial, int nsplit, cudaStream_t st,
-                        int mirror_z_origin)
+                        int mirror_z_origin, const float *sino_ci, int ci_groups)
 {
     const bool pair = mirror_z_origin != CBCT_NO_MIRROR_PAIR;
     if (pair && (!g->sym_mirror_z || zs1 > (g->d.vol_nz + 1) / 2)) return CBCT_ERR_INVALID_ARG;
@@ -554,12 +591,12 @@ int cbct_launch_adjoint(cbct_geom *g, const float *sino_src, float *vol, int cha
     G.nq = 0;
     const size_t sstride = (size_t)d.n_views * d.det_nv * d.det_nu;
     if (NR == 4) {
-        return mirror ? launch_gather_channels<4, 2>(g, G, sino_src, vol, channels, sstride, vol_channel_stride, vol_z_origin, partial, nsplit, st)
-                      : launch_gather_channels<4, 1>(g, G, sino_src, vol, channels, sstride, vol_channel_stride, vol_z_origin, partial, nsplit, st);
+        return mirror ? launch_gather_channels<4, 2>(g, G, sino_src, vol, channels, sstride, vol_channel_stride, vol_z_origin, partial, nsplit, st, sino_ci, ci_groups)
+                      : launch_gather_channels<4, 1>(g, G, sino_src, vol, channels, sstride, vol_channel_stride, vol_z_origin, partial, nsplit, st, sino_ci, ci_groups);
     } else if (NR == 2) {
-        return mirror ? launch_gather_channels<2, 2>(g, G, sino_src, vol, channels, sstride, vol_channel_stride, vol_z_origin, partial, nsplit, st)
-                      : launch_gather_channels<2, 1>(g, G, sino_src, vol, channels, sstride, vol_channel_stride, vol_z_origin, partial, nsplit, st);
+        return mirror ? launch_gather_channels<2, 2>(g, G, sino_src, vol, channels, sstride, vol_channel_stride, vol_z_origin, partial, nsplit, st, sino_ci, ci_groups)
+                      : launch_gather_channels<2, 1>(g, G, sino_src, vol, channels, sstride, vol_channel_stride, vol_z_origin, partial, nsplit, st, sino_ci, ci_groups);
     }
-    return mirror ? launch_gather_channels<1, 2>(g, G, sino_src, vol, channels, sstride, vol_channel_stride, vol_z_origin, partial, nsplit, st)
-                  : launch_gather_channels<1, 1>(g, G, sino_src, vol, channels, sstride, vol_channel_stride, vol_z_origin, partial, nsplit, st);
+    return mirror ? launch_gather_channels<1, 2>(g, G, sino_src, vol, channels, sstride, vol_channel_stride, vol_z_origin, partial, nsplit, st, sino_ci, ci_groups)
+                  : launch_gather_channels<1, 1>(g, G, sino_src, vol, channels, sstride, vol_channel_stride, vol_z_origin, partial, nsplit, st, sino_ci, ci_groups);
 }

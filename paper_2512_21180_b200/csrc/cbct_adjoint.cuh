@@ -32,7 +32,8 @@ struct AdjGeom {
 // column-walk kernel (cbct_adjoint_column.cu): returns CBCT_OK after launching, or 1 if this geometry / channel block
 // is not one it serves (the caller then takes the voxel kernel).  CB channels starting at sinoI / vol.
 // `partial` (nsplit > 1): workspace of nsplit * CB * nx * ny * nz floats for the partial outputs of the view groups.
-int cbct_launch_adjoint_column(cbct_geom *g, AdjGeom &G, int NR, int NM, int CB, const float *sinoI, float *vol,
+// CI = 4: sinoI points at channel-interleaved groups of 4 (NR = 1 only; CB = 4, or 8 with NM = 1), else CI = 1.
+int cbct_launch_adjoint_column(cbct_geom *g, AdjGeom &G, int NR, int NM, int CB, int CI, const float *sinoI, float *vol,
                                size_t sstride, size_t vstride, int vol_z_origin, float *partial, int nsplit,
                                cudaStream_t st);
 // out[c][e] = sum_s partial[s][c][e], fixed order (cbct_adjoint.cu)

@@ -31,7 +31,10 @@
 #endif
 #define ADJC_NT (ADJ_BX * ADJC_BY)
 
-template <int NR, int NM, int CB, int ZC, int MINB>
+// CI = 4 (only with NR = 1): the channels come interleaved in groups of 4 -- record (view, iv, iu) of group gq holds
+// the pixel of channels 4 gq .. 4 gq + 3, one LDG.128 (cbct_launch_interleave_channels) -- instead of CB scalar loads
+// from CB planar sinograms; `sino_cstride` stays the planar channel stride, a group spans 4 of them.
+template <int NR, int NM, int CB, int ZC, int MINB, int CI = 1>
 __global__ void __launch_bounds__(ADJC_NT, MINB)
 adjoint_column_kernel(const float *__restrict__ sinoI, float *__restrict__ vol, const __grid_constant__ AdjGeom G,
                       const __grid_constant__ ViewChunk V, int q0, int accumulate, size_t sino_cstride,
@@ -93,7 +96,7 @@ adjoint_column_kernel(const float *__restrict__ sinoI, float *__restrict__ vol, 
         const float dNx = -sf * duf, dNy = cf * duf;
         const float Ax_lo = -sf * au_lo, Ay_lo = cf * au_lo, dAx = -sf * lu, dAy = cf * lu;
         const int a = (q0 + q) / G.nbase, ib = (q0 + q) - a * G.nbase;
-        const float *sq = sinoI + (size_t)ib * img * NR;
+        const float *sq = sinoI + (size_t)ib * img * (NR * CI);
 
         // sliding window: R[j] = this view's sums of plane tw + j (relative to zc0), by stored component
         float R[3][NA][NR];
@@ -150,16 +153,31 @@ adjoint_column_kernel(const float *__restrict__ sinoI, float *__restrict__ vol, 
             if (last) break;
             const float fb = av0 - t0f;    // f at mu = 0, in [zb, 1 + zb)
             const float L2row = fmaf(v, v, sdd2f);
-            const float *row0 = sq + iv * G.nu * NR, *row1 = sq + (G.nv - 1 - iv) * G.nu * NR;
+            const float *row0 = sq + iv * G.nu * (NR * CI), *row1 = sq + (G.nv - 1 - iv) * G.nu * (NR * CI);
             float u = u_lo, Nx = Nx_lo, Ny = Ny_lo, Ax = Ax_lo, Ay = Ay_lo;
 
             for (int iu = iu_lo; iu <= iu_hi; ++iu, u += duf, Nx += dNx, Ny += dNy, Ax += dAx, Ay += dAy) {
                 // the pixel loads go first: the weight arithmetic below covers their latency
                 float y0[CB][NR], y1[NM == 2 ? CB : 1][NR];
+                if constexpr (CI == 4) {
 #pragma unroll
-                for (int cc = 0; cc < CB; ++cc) {
-                    load_views<NR>(row0 + cc * sino_cstride + iu * NR, y0[cc]);
-                    if (NM == 2) load_views<NR>(row1 + cc * sino_cstride + iu * NR, y1[cc]);
+                    for (int gq = 0; gq < CB / 4; ++gq) {
+                        float t[4];
+                        load_views<4>(row0 + gq * 4 * sino_cstride + iu * 4, t);
+#pragma unroll
+                        for (int k = 0; k < 4; ++k) y0[gq * 4 + k][0] = t[k];
+                        if (NM == 2) {
+                            load_views<4>(row1 + gq * 4 * sino_cstride + iu * 4, t);
+#pragma unroll
+                            for (int k = 0; k < 4; ++k) y1[NM == 2 ? gq * 4 + k : 0][0] = t[k];
+                        }
+                    }
+                } else {
+#pragma unroll
+                    for (int cc = 0; cc < CB; ++cc) {
+                        load_views<NR>(row0 + cc * sino_cstride + iu * NR, y0[cc]);
+                        if (NM == 2) load_views<NR>(row1 + cc * sino_cstride + iu * NR, y1[cc]);
+                    }
                 }
                 // window of mu from the dominant horizontal axis: |A_d + mu N_d| < 1
                 const bool domx = fabsf(Nx) >= fabsf(Ny);
@@ -249,7 +267,7 @@ adjoint_column_kernel(const float *__restrict__ sinoI, float *__restrict__ vol, 
 #define ADJC_FLOATS 64
 #endif
 
-template <int NR, int NM, int CB>
+template <int NR, int NM, int CB, int CI = 1>
 static int launch_column(cbct_geom *g, AdjGeom &G, const float *sinoI, float *vol, size_t sstride, size_t vstride,
                          int vol_z_origin, float *partial, int nsplit, cudaStream_t st)
 {
@@ -259,7 +277,7 @@ static int launch_column(cbct_geom *g, AdjGeom &G, const float *sinoI, float *vo
 #define ADJC_MINB 0
 #endif
     constexpr int MINB = ADJC_MINB;
-    auto kernel = adjoint_column_kernel<NR, NM, CB, ZC, MINB>;
+    auto kernel = adjoint_column_kernel<NR, NM, CB, ZC, MINB, CI>;
     const size_t smem = (size_t)ZC * NACC * ADJC_NT * sizeof(float);
     const int nq_total = g->d.n_views;
     G.nbase = g->d.n_views / NR;
@@ -320,14 +338,19 @@ static int launch_column(cbct_geom *g, AdjGeom &G, const float *sinoI, float *vo
 }
 
 template <int NR, int NM>
-static int launch_column_cb(cbct_geom *g, AdjGeom &G, int CB, const float *sinoI, float *vol, size_t sstride,
+static int launch_column_cb(cbct_geom *g, AdjGeom &G, int CB, int CI, const float *sinoI, float *vol, size_t sstride,
                             size_t vstride, int vol_z_origin, float *partial, int nsplit, cudaStream_t st)
 {
+    if (CI != 1 && !(CI == 4 && NR == 1 && (CB == 4 || (CB == 8 && NM == 1)))) return CBCT_ERR_INVALID_ARG;
     // the partial outputs of the view groups take nsplit * CB volumes: at most 16 (cbct_adjoint_partial_floats)
     if (nsplit * CB > 16) nsplit = 16 / CB;
     if (CB == 1) return launch_column<NR, NM, 1>(g, G, sinoI, vol, sstride, vstride, vol_z_origin, partial, nsplit, st);
     if (CB == 2) return launch_column<NR, NM, 2>(g, G, sinoI, vol, sstride, vstride, vol_z_origin, partial, nsplit, st);
     // geometries with few symmetric images fill the window's 8 accumulators per plane with channels instead
+    if constexpr (NR == 1) {
+        if (CB == 4 && CI == 4) return launch_column<NR, NM, 4, 4>(g, G, sinoI, vol, sstride, vstride, vol_z_origin, partial, nsplit, st);
+        if (CB == 8 && CI == 4 && NM == 1) return launch_column<NR, 1, 8, 4>(g, G, sinoI, vol, sstride, vstride, vol_z_origin, partial, nsplit, st);
+    }
     if constexpr (NR * NM <= 2) {
         if (CB == 4) return launch_column<NR, NM, 4>(g, G, sinoI, vol, sstride, vstride, vol_z_origin, partial, nsplit, st);
     }
@@ -337,17 +360,17 @@ static int launch_column_cb(cbct_geom *g, AdjGeom &G, int CB, const float *sinoI
     return 1;
 }
 
-int cbct_launch_adjoint_column(cbct_geom *g, AdjGeom &G, int NR, int NM, int CB, const float *sinoI, float *vol,
+int cbct_launch_adjoint_column(cbct_geom *g, AdjGeom &G, int NR, int NM, int CB, int CI, const float *sinoI, float *vol,
                                size_t sstride, size_t vstride, int vol_z_origin, float *partial, int nsplit,
                                cudaStream_t st)
 {
     // preconditions of the three-plane identity and of the 6-sample window (see the header): f < 2 needs
     // 2 zb = 2 sqrt 2 |v| / sdd < 1 on every detector row; longer windows take the voxel kernel's walking variant
     if (G.fine || !(G.tz < 0.35f)) return 1;
-    if (NR == 4) return NM == 2 ? launch_column_cb<4, 2>(g, G, CB, sinoI, vol, sstride, vstride, vol_z_origin, partial, nsplit, st)
-                                : launch_column_cb<4, 1>(g, G, CB, sinoI, vol, sstride, vstride, vol_z_origin, partial, nsplit, st);
-    if (NR == 2) return NM == 2 ? launch_column_cb<2, 2>(g, G, CB, sinoI, vol, sstride, vstride, vol_z_origin, partial, nsplit, st)
-                                : launch_column_cb<2, 1>(g, G, CB, sinoI, vol, sstride, vstride, vol_z_origin, partial, nsplit, st);
-    return NM == 2 ? launch_column_cb<1, 2>(g, G, CB, sinoI, vol, sstride, vstride, vol_z_origin, partial, nsplit, st)
-                   : launch_column_cb<1, 1>(g, G, CB, sinoI, vol, sstride, vstride, vol_z_origin, partial, nsplit, st);
+    if (NR == 4) return NM == 2 ? launch_column_cb<4, 2>(g, G, CB, CI, sinoI, vol, sstride, vstride, vol_z_origin, partial, nsplit, st)
+                                : launch_column_cb<4, 1>(g, G, CB, CI, sinoI, vol, sstride, vstride, vol_z_origin, partial, nsplit, st);
+    if (NR == 2) return NM == 2 ? launch_column_cb<2, 2>(g, G, CB, CI, sinoI, vol, sstride, vstride, vol_z_origin, partial, nsplit, st)
+                                : launch_column_cb<2, 1>(g, G, CB, CI, sinoI, vol, sstride, vstride, vol_z_origin, partial, nsplit, st);
+    return NM == 2 ? launch_column_cb<1, 2>(g, G, CB, CI, sinoI, vol, sstride, vstride, vol_z_origin, partial, nsplit, st)
+                   : launch_column_cb<1, 1>(g, G, CB, CI, sinoI, vol, sstride, vstride, vol_z_origin, partial, nsplit, st);
 }

@@ -394,12 +394,25 @@ static int adjoint_impl(const cbct_geom *gc, const float *sino, float *vol, int3
         rc = cbct_launch_interleave_views(g, d_sino, g->ws_sino2, channels, weighted ? g->d_filter_tab : nullptr, st);
         if (rc) return rc;
         d_sino = g->ws_sino2;
-    } else if (weighted) {  // no re-layout pass to fuse into: one weighting pass into workspace
-        rc = ensure(&g->ws_sino2, &g->ws_sino2_bytes, sino_bytes);
+    }
+    // no rotation symmetry: channels interleaved in groups of 4 for the column kernel's vector loads (w(u) fused into
+    // that pass), and, if weighted, one weighting pass for the channels and kernels that read the planar layout
+    const float *sino_ci = nullptr;
+    const int ci_groups = g->sym_rot == 1 ? cbct_adjoint_channel_groups(g, channels, cx.kv == MEM_DEVICE) : 0;
+    if (g->sym_rot == 1 && (weighted || ci_groups)) {
+        const size_t plain = weighted ? cx.nsino * channels : 0, grouped = (size_t)ci_groups * 4 * cx.nsino;
+        rc = ensure(&g->ws_sino2, &g->ws_sino2_bytes, (plain + grouped) * sizeof(float));
         if (rc) return rc;
-        rc = cbct_launch_redundancy_weight(g, d_sino, g->ws_sino2, channels, st);
-        if (rc) return rc;
-        d_sino = g->ws_sino2;
+        if (ci_groups) {
+            rc = cbct_launch_interleave_channels(g, d_sino, g->ws_sino2 + plain, ci_groups, weighted ? g->d_filter_tab : nullptr, st);
+            if (rc) return rc;
+            sino_ci = g->ws_sino2 + plain;
+        }
+        if (weighted) {
+            rc = cbct_launch_redundancy_weight(g, d_sino, g->ws_sino2, channels, st);
+            if (rc) return rc;
+            d_sino = g->ws_sino2;
+        }
     }
     // the views of a launch split over groups of CTAs (partial outputs in workspace, then reduced)
     int nsplit = cx.kv == MEM_DEVICE ? cbct_adjoint_view_splits(g) : 1;
@@ -410,7 +423,8 @@ static int adjoint_impl(const cbct_geom *gc, const float *sino, float *vol, int3
         partial = g->ws_vol;
     }
     rc = produce_volume(cx, vol, g->sym_mirror_z != 0, [&](float *dst, int zs0, int zs1, size_t cstride, int z_origin, int mirror_origin) {
-        return cbct_launch_adjoint(g, d_sino, dst, channels, zs0, zs1, cstride, z_origin, partial, nsplit, st, mirror_origin);
+        return cbct_launch_adjoint(g, d_sino, dst, channels, zs0, zs1, cstride, z_origin, partial, nsplit, st, mirror_origin,
+                                   sino_ci, ci_groups);
     });
     if (rc) return rc;
     if (cx.pageable) CBCT_CUDA_TRY(cudaStreamSynchronize(st));
@@ -553,7 +567,9 @@ extern "C" int cbct_geom_reserve(cbct_geom *g, int32_t channels)
     if (rc) return rc;
     // backprojectors: re-laid-out sinogram (view-interleaved / zero-bordered)
     const size_t psino = cbct_padded_sino_floats(g);
-    rc = ensure(&g->ws_sino2, &g->ws_sino2_bytes, (psino > nsino ? psino : nsino) * channels * sizeof(float));
+    // (sym_rot == 1: the weighted adjoint keeps a weighted planar copy beside the channel groups)
+    const size_t adj_sino = g->sym_rot == 1 ? 2 * nsino : nsino;
+    rc = ensure(&g->ws_sino2, &g->ws_sino2_bytes, (psino > adj_sino ? psino : adj_sino) * channels * sizeof(float));
     if (rc) return rc;
     return cbct_ensure_filter_tables(g);
 }

@@ -122,9 +122,14 @@ int cbct_ensure_filter_tables(cbct_geom *g);
 int cbct_launch_negate(cbct_geom *g, float *buf, size_t n, cudaStream_t st);  // buf = -buf (cbct_fp.cu)
 int cbct_launch_redundancy_weight(cbct_geom *g, const float *in, float *out, int channels, cudaStream_t st);
 // gather adjoint into vol planes [zs0, zs1)
+// sino_ci / ci_groups (sym_rot == 1 only, else nullptr / 0): channels [0, 4 ci_groups) also given interleaved in
+// groups of 4 (cbct_launch_interleave_channels), which the column kernel reads with one vector load per pixel
 int cbct_launch_adjoint(cbct_geom *g, const float *sino_src, float *vol, int channels, int zs0, int zs1,
                         size_t vol_channel_stride, int vol_z_origin, float *partial, int nsplit, cudaStream_t st,
-                        int mirror_z_origin = CBCT_NO_MIRROR_PAIR);
+                        int mirror_z_origin = CBCT_NO_MIRROR_PAIR, const float *sino_ci = nullptr, int ci_groups = 0);
+int cbct_adjoint_channel_groups(const cbct_geom *g, int channels, bool device_volume);
+int cbct_launch_interleave_channels(cbct_geom *g, const float *sino, float *out, int groups, const float *weights,
+                                    cudaStream_t st);
 int cbct_adjoint_view_splits(const cbct_geom *g);   // view groups per tile of the adjoint (1 = none)
 bool cbct_adjoint_small_grid(const cbct_geom *g);    // fewer than 2 million base voxels: the voxel kernel splits views
 size_t cbct_adjoint_partial_floats(const cbct_geom *g);  // workspace floats of the view groups' partial outputs
