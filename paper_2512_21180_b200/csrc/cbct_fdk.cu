@@ -79,8 +79,10 @@ struct FdkViews {
 // 1.5e-5 px ulp of a raw fp32 coordinate near 256 (DESIGN.md s.6).
 // CB channels per thread share the whole per-(x, y, view) set-up (the fp64 coordinates, the weight) and the
 // per-voxel row arithmetic; their records lie `sino_cstride` float4 apart.
-template <int NR, int NM, int ZB, int CB>
-__global__ void __launch_bounds__(FDK_BX *FDK_BY)
+// MB = CTAs per SM the register allocation aims for (0: the compiler's choice).  Not for occupancy's sake: the bound
+// decides how many of a view's loads ptxas keeps in flight ahead of their use, and the kernel waits on its loads.
+template <int NR, int NM, int ZB, int CB, int MB>
+__global__ void __launch_bounds__(FDK_BX *FDK_BY, MB)
 fdk_kernel(const float *__restrict__ sinoP, float *__restrict__ vol, const __grid_constant__ FdkGeom G,
            const __grid_constant__ FdkViews V, int q0, int accumulate, int vol_z_origin, size_t sino_cstride,
            size_t vol_cstride)
@@ -234,7 +236,7 @@ int cbct_launch_pad_sino(cbct_geom *g, const float *src, float *dst, int channel
 #define FDK_CB 2
 #endif
 
-template <int NR, int NM, int ZB>
+template <int NR, int NM, int ZB, int MB = 0, int MB2 = MB>
 static int launch_fdk(cbct_geom *g, FdkGeom &G, const float *padded, float *vol, int channels, size_t vstride,
                       int vol_z_origin, cudaStream_t st)
 {
@@ -254,11 +256,11 @@ static int launch_fdk(cbct_geom *g, FdkGeom &G, const float *padded, float *vol,
         while (c < channels) {
             cbct_prof_begin(g, CBCT_KERNEL_FDK, st);
             if (FDK_CB >= 2 && NR == 1 && channels - c >= 2) {
-                fdk_kernel<NR, NM, ZB, 2><<<grid, block, 0, st>>>(rec + c * sstride, vol + c * vstride, G, fv, q0, q0 > 0,
+                fdk_kernel<NR, NM, ZB, 2, MB2><<<grid, block, 0, st>>>(rec + c * sstride, vol + c * vstride, G, fv, q0, q0 > 0,
                                                                   vol_z_origin, sstride, vstride);
                 c += 2;
             } else {
-                fdk_kernel<NR, NM, ZB, 1><<<grid, block, 0, st>>>(rec + c * sstride, vol + c * vstride, G, fv, q0, q0 > 0,
+                fdk_kernel<NR, NM, ZB, 1, MB><<<grid, block, 0, st>>>(rec + c * sstride, vol + c * vstride, G, fv, q0, q0 > 0,
                                                                   vol_z_origin, sstride, vstride);
                 c += 1;
             }
@@ -304,10 +306,14 @@ int cbct_launch_fdk(cbct_geom *g, const float *padded_sino, float *vol, int chan
     G.n_views = 0; G.nbase = 0;
     const size_t vs = vol_channel_stride;
     // z per thread: 3 measured best for the 8-voxel variant (1: 6.3 ms, 2: 4.8, 3: 4.6, 4: 5.2, 8: 5.3 per channel)
-    if (NR == 4) return mirror ? launch_fdk<4, 2, 3>(g, G, padded_sino, vol, channels, vs, vol_z_origin, st)
+    // planes per thread and register bound per instance, measured at 256^3 / 400 views (ms per channel; the bound
+    // steers how many loads ptxas keeps in flight, see fdk_kernel): NR 4 / NM 2: 3 planes, bound 7: 4.48 (no bound
+    // 4.62; 2 planes 4.75, 4: 4.51, 8: 5.6);  NR 2 / NM 2: 8 planes, bound 4: 4.95 (no bound 6.11);  NR 1 / NM 2:
+    // 8 planes, bound 7: 5.60 (no bound 6.80), two channels per thread with bound 4: 4.64 per channel.
+    if (NR == 4) return mirror ? launch_fdk<4, 2, 3, 7>(g, G, padded_sino, vol, channels, vs, vol_z_origin, st)
                                : launch_fdk<4, 1, 8>(g, G, padded_sino, vol, channels, vs, vol_z_origin, st);
-    if (NR == 2) return mirror ? launch_fdk<2, 2, 8>(g, G, padded_sino, vol, channels, vs, vol_z_origin, st)
+    if (NR == 2) return mirror ? launch_fdk<2, 2, 8, 4>(g, G, padded_sino, vol, channels, vs, vol_z_origin, st)
                                : launch_fdk<2, 1, 8>(g, G, padded_sino, vol, channels, vs, vol_z_origin, st);
-    return mirror ? launch_fdk<1, 2, 8>(g, G, padded_sino, vol, channels, vs, vol_z_origin, st)
+    return mirror ? launch_fdk<1, 2, 8, 7, 4>(g, G, padded_sino, vol, channels, vs, vol_z_origin, st)
                   : launch_fdk<1, 1, 8>(g, G, padded_sino, vol, channels, vs, vol_z_origin, st);
 }
