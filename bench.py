@@ -438,8 +438,11 @@ def main():
     # 4.05 cycles, profiles/r1_l1_microbench.md) x the SM clock sampled during the timed region; FP32 issue 148 SMs x
     # 128 lanes x that clock (measured 3.89 of 4 warp-instructions per clock per SM, profiles/r2_microbench.md)
     quarter_turns = rotations == 4 and cfg["vol_nx"] == cfg["vol_ny"]
+    # channels outside a group of 4: their quarter-turn images (fp4_pair_kernel), else mirror-paired cells (fpm_kernel)
+    # on z-symmetric geometries held resident, else quad-packed cells (fp_kernel)
+    tail_kernel = "fpm_kernel" if (mirror and not streamed) else "fp_kernel"
     names = {"fp": ("fp4_pair_kernel" if (C % 4 == 0 or quarter_turns)
-                    else ("fp_kernel" if C < 4 else "fp4_pair_kernel+fp_kernel")),
+                    else (tail_kernel if C < 4 else "fp4_pair_kernel+" + tail_kernel)),
              "adjoint": None, "fdk": "fdk_kernel"}
     # adjoint (cbct_adjoint.cu: launch_gather_channels), on grids of 2 million base voxels or more: with rotation
     # symmetry, blocks of 4 (or 8) channels take the voxel kernel and the remaining 1-3 channels the column-walk kernel;

@@ -320,6 +320,108 @@ fp4_pair_kernel(const float4 *__restrict__ packed, float *__restrict__ sino, con
     *dst2 = accumulate ? *dst2 + val2 : val2;
 }
 
+// ---------------------------------------------------------------------------
+// Single channels on geometries that are symmetric under z -> -z but have no quarter-turn symmetry between their views
+// (irregular angle lists): "mirror-paired" cells.  The ray to pixel (iu, nv-1-iv) is the mirror image of the ray to
+// (iu, iv): same length, same sample lattice, same x and y, z -> -z; its trilinear sample has the same cell and the
+// same fractions when it is read from the mirrored volume f_M[z] = f[nz-1-z].  A cell holds
+//     float4( f[z][y][x], f[z][y][x+1], f_M[z][y][x], f_M[z][y][x+1] )
+// for the planes of the LOWER half only (rays with v <= 0 never rise above the mid-plane), in the skewed rows of the
+// channel-interleaved layout.  One thread walks the ray of a lower detector row and accumulates both it and its
+// mirror image: 4 LDG.128 (the y, z corners; the x pair sits inside the cell) per PAIR of samples -- as many loads
+// per sample as the quad-packed layout, but the position / fraction / address arithmetic is shared by the pair
+// (the quad-packed kernel is as much issue-bound, 78 % of its slots, as L1-bound) and the volume's bytes a beam
+// pulls through L1 are halved (every voxel stored twice instead of four times).
+// ---------------------------------------------------------------------------
+static int fpm_ztop(int nz) { return (nz + 1) / 2 + 1; }   // highest plane held, inclusive (one above the samples' reach)
+
+__global__ void __launch_bounds__(256)
+pack_volume_mirror_kernel(const float *__restrict__ src, float4 *__restrict__ dst, const __grid_constant__ RayGeom G,
+                          size_t src_cstride, size_t dst_cstride)
+{
+    // G: the geometry of the lower slab, planes [0, G.z1) of a grid of G.nz planes
+    const float *s = src + (size_t)blockIdx.z * src_cstride;
+    float4 *d = dst + (size_t)blockIdx.z * dst_cstride;
+    const int pitch = G.px + CBCT_ROW_SKEW;
+    const int pos = blockIdx.x * blockDim.x + threadIdx.x;
+    if (pos >= pitch) return;
+    for (int row = blockIdx.y; row < G.py * G.pz; row += gridDim.y) {
+        const int jy = row % G.py, jz = row / G.py;
+        const int x = pos - ((CBCT_SWIZZLE_Y * jy + CBCT_SWIZZLE_Z * jz) & 7) - CBCT_PAD;
+        const int y = jy - CBCT_PAD, z = jz - CBCT_PAD, zm = G.nz - 1 - z;
+        float4 q = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (y >= 0 && y < G.ny) {
+            const bool x0 = x >= 0 && x < G.nx, x1 = x + 1 >= 0 && x + 1 < G.nx;
+            if (z >= 0 && z < G.nz) {
+                const float *p = s + ((size_t)z * G.ny + y) * G.nx + x;
+                if (x0) q.x = __ldg(p);
+                if (x1) q.y = __ldg(p + 1);
+            }
+            if (zm >= 0 && zm < G.nz) {
+                const float *p = s + ((size_t)zm * G.ny + y) * G.nx + x;
+                if (x0) q.z = __ldg(p);
+                if (x1) q.w = __ldg(p + 1);
+            }
+        }
+        d[(size_t)row * pitch + pos] = q;
+    }
+}
+
+__device__ __forceinline__ void fpm_sample(const float4 *__restrict__ packed, const Ray &r, float kf, unsigned py,
+                                           unsigned pitch, unsigned plane, unsigned kfold, float &A, float &M)
+{
+    const float yx = fmaf(kf, r.dx, r.ax) + CBCT_MAGIC;
+    const float yy = fmaf(kf, r.dy, r.ay) + CBCT_MAGIC;
+    const float yz = fmaf(kf, r.dz, r.az) + CBCT_MAGIC;
+    const float fx = fmaf(kf, r.dx, r.bx - (yx - CBCT_MAGIC));
+    const float fy = fmaf(kf, r.dy, r.by - (yy - CBCT_MAGIC));
+    const float fz = fmaf(kf, r.dz, r.bz - (yz - CBCT_MAGIC));
+    const unsigned ux = __float_as_uint(yx), uy = __float_as_uint(yy), uz = __float_as_uint(yz);
+    const unsigned t = uy * CBCT_SWIZZLE_Y + uz * CBCT_SWIZZLE_Z;  // magic bits are multiples of 8
+    const unsigned base = (uz * py + uy) * pitch + ux - kfold;
+    const float4 c00 = __ldg(packed + (base + (t & 7u)));
+    const float4 c10 = __ldg(packed + (base + pitch + ((t + CBCT_SWIZZLE_Y) & 7u)));
+    const float4 c01 = __ldg(packed + (base + plane + ((t + CBCT_SWIZZLE_Z) & 7u)));
+    const float4 c11 = __ldg(packed + (base + plane + pitch + ((t + CBCT_SWIZZLE_Y + CBCT_SWIZZLE_Z) & 7u)));
+    const float gy = 1.0f - fy, gz = 1.0f - fz;
+    const float w00 = gy * gz, w10 = fy * gz, w01 = gy * fz, w11 = fy * fz;
+    A += fmaf(w00, lerpf(c00.x, c00.y, fx), fmaf(w10, lerpf(c10.x, c10.y, fx), fmaf(w01, lerpf(c01.x, c01.y, fx), w11 * lerpf(c11.x, c11.y, fx))));
+    M += fmaf(w00, lerpf(c00.z, c00.w, fx), fmaf(w10, lerpf(c10.z, c10.w, fx), fmaf(w01, lerpf(c01.z, c01.w, fx), w11 * lerpf(c11.z, c11.w, fx))));
+}
+
+// G: geometry of the lower slab (planes [0, G.z1)); nvh = rows with v <= 0 = ceil(nv / 2); CTA as fp_kernel
+template <int TU>
+__global__ void __launch_bounds__(32 * (FP_CTA_U / TU) * FPK_VPC)
+fpm_kernel(const float4 *__restrict__ packed, float *__restrict__ sino, const __grid_constant__ RayGeom G,
+           const __grid_constant__ ViewChunk V, int view0, int accumulate, int nvh, const float *__restrict__ sub,
+           int nviews)
+{
+    constexpr int TV = 32 / TU, WU = FP_CTA_U / TU;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int iu = blockIdx.x * FP_CTA_U + (warp % WU) * TU + (lane % TU);
+    const int iv = blockIdx.z * TV + (lane / TU);
+    const int view = blockIdx.y * FPK_VPC + warp / WU;
+    if (iu >= G.nu || iv >= nvh || view >= nviews) return;
+    const Ray r = cbct_ray_setup(G, V.cs[view].x, V.cs[view].y, iu, iv);
+    const unsigned py = G.py, pitch = G.px + CBCT_ROW_SKEW, plane = pitch * py;
+    const unsigned kfold = CBCT_MAGIC_BITS * ((py + 1u) * pitch + 1u);
+    float a0 = 0.f, a1 = 0.f, m0 = 0.f, m1 = 0.f;
+    float kf = r.kf0;
+    int it = 0;
+    for (; it + 1 < r.n; it += 2, kf += 2.0f) {
+        fpm_sample(packed, r, kf, py, pitch, plane, kfold, a0, m0);
+        fpm_sample(packed, r, kf + 1.0f, py, pitch, plane, kfold, a1, m1);
+    }
+    if (it < r.n) fpm_sample(packed, r, kf, py, pitch, plane, kfold, a0, m0);
+    const float delta = (float)G.delta;
+    const int ivm = G.nv - 1 - iv;
+    const size_t o = ((size_t)(view0 + view) * G.nv + iv) * G.nu + iu, om = ((size_t)(view0 + view) * G.nv + ivm) * G.nu + iu;
+    float val = (a0 + a1) * delta, valm = (m0 + m1) * delta;
+    if (sub) { val -= __ldg(sub + o); valm -= __ldg(sub + om); }
+    sino[o] = accumulate ? sino[o] + val : val;
+    if (ivm != iv) sino[om] = accumulate ? sino[om] + valm : valm;   // the middle row of an odd nv is its own image
+}
+
 __global__ void __launch_bounds__(256) negate_kernel(float *buf, size_t n)
 {
     for (size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x; e < n; e += (size_t)gridDim.x * blockDim.x)
@@ -336,6 +438,15 @@ size_t cbct_packed_volume_cells(const RayGeom &r) { return (size_t)r.px * r.py *
 static size_t packed_tail_offset(const RayGeom &r, int channels) { return (size_t)(channels / 4) * cbct_packed4_cells(r); }
 // channels left over by the groups of 4: their quarter-turn images when the geometry has that symmetry
 static bool tail_by_rotation(const cbct_geom *g, const RayGeom &r) { return g->sym_rot == 4 && r.nx == r.ny; }
+// geometry of the lower slab that the mirror-paired layout holds (planes [0, fpm_ztop] of the whole grid)
+static RayGeom mirror_raygeom(const cbct_geom *g) { return cbct_make_raygeom(g, 0, fpm_ztop(g->d.vol_nz) + 1); }
+// ... used for the channels left over by the groups of 4 when the whole volume is resident (a z-slab of a streamed
+// call does not hold its mirror planes) and the slab is no larger than the quad-packed one the workspace is sized for
+static bool tail_by_mirror(const cbct_geom *g, const RayGeom &r)
+{
+    if (tail_by_rotation(g, r) || !g->sym_mirror_z || r.z0 != 0 || r.z1 != r.nz || r.nz < 8) return false;
+    return cbct_packed4_cells(mirror_raygeom(g)) <= cbct_packed_volume_cells(r);
+}
 size_t cbct_packed_tail_cells(const cbct_geom *g, const RayGeom &r)
 {
     return tail_by_rotation(g, r) ? cbct_packed4_cells(r) : cbct_packed_volume_cells(r);
@@ -359,6 +470,15 @@ int cbct_launch_pack_volume(cbct_geom *g, const RayGeom &r, const float *src, fl
                                                       dst + packed_tail_offset(r, channels), r, src_channel_stride,
                                                       src_z_origin, cbct_packed4_cells(r));
         return cbct_check_launch(g, "pack_volume_rot4_kernel");
+    }
+    if (tail && tail_by_mirror(g, r)) {
+        const RayGeom rm = mirror_raygeom(g);
+        const int rows_m = rm.py * rm.pz;
+        dim3 grid((rm.px + CBCT_ROW_SKEW + 255) / 256, rows_m < 148 * 8 ? rows_m : 148 * 8, tail);
+        pack_volume_mirror_kernel<<<grid, 256, 0, st>>>(src + (size_t)4 * groups * src_channel_stride + (size_t)(0 - src_z_origin) * r.ny * r.nx,
+                                                        dst + packed_tail_offset(r, channels), rm, src_channel_stride,
+                                                        cbct_packed_volume_cells(r));
+        return cbct_check_launch(g, "pack_volume_mirror_kernel");
     }
     if (tail) {
         dim3 grid((r.px + 255) / 256, gy, tail);
@@ -462,6 +582,20 @@ int cbct_launch_fp(cbct_geom *g, const RayGeom &r, const float4 *packed, float *
             if (rc) return rc;
         }
         const float4 *tail = packed + packed_tail_offset(r, channels) - (size_t)c * pstride;
+        if (c < channels && !rot_tail && tail_by_mirror(g, r)) {
+            // leftover channels one by one through the mirror-paired cells: the rows with v <= 0, each with its image
+            const RayGeom rm = mirror_raygeom(g);
+            const int nvh = (r.nv + 1) / 2;
+            dim3 grid((r.nu + FP_CTA_U - 1) / FP_CTA_U, (n + FPK_VPC - 1) / FPK_VPC, (nvh + 7) / 8);
+            for (; c < channels; ++c) {
+                cbct_prof_begin(g, CBCT_KERNEL_FP, st);
+                fpm_kernel<4><<<grid, 32 * (FP_CTA_U / 4) * FPK_VPC, 0, st>>>(tail + c * pstride, sino + c * sstride, rm, vc, view0,
+                                                                              accumulate, nvh, sub ? sub + c * sstride : nullptr, n);
+                cbct_prof_end(g, CBCT_KERNEL_FP, st);
+                int rc = cbct_check_launch(g, "fpm_kernel");
+                if (rc) return rc;
+            }
+        }
         while (c < channels && !rot_tail) {
             int left = channels - c, rc;
             const float4 *p = tail + c * pstride;

@@ -852,6 +852,37 @@ def test_fp_channel_groups(cbct, oracle_mod, C, cap, over):
     assert np.max(np.abs(got - (ref - y))) <= 2e-5 * scale
 
 
+@pytest.mark.parametrize("over,C", [
+    (dict(n_views=7), 1),                                                   # odd view count: no rotation, z-mirror
+    (dict(n_views=9, irregular=True, det_off_u_mm=20.0), 3),                # irregular angles, half-fan, 3 channels
+    (dict(n_views=8, irregular=True, det_nv=47, vol_nz=27), 2),             # odd detector rows (a row is its own image), odd nz
+    (dict(n_views=10, vol_nx=30, det_nu=50), 5),                            # two-fold rotation only: group of 4 + 1
+    (dict(n_views=530, irregular=True, vol_nx=16, vol_ny=16, vol_nz=12, det_nu=20, det_nv=18, det_du_mm=6.0,
+          det_dv_mm=6.0), 1),                                               # more views than one launch chunk
+])
+def test_fp_mirror_paired_cells(cbct, oracle_mod, over, C):
+    """Channels outside a group of 4 on z-symmetric geometries without the quarter-turn symmetry go through the
+    mirror-paired cells (fpm_kernel: a thread walks the ray of a lower detector row together with its mirror image).
+    Whole sinogram against the oracle, with and without the fused residual (R3, R4)."""
+    kw, extra = _symmetry_case(over)
+    if "angles_rad" in extra:
+        extra["angles_rad"] = list(np.sort(np.random.default_rng(8).uniform(0, 2 * np.pi, kw["n_views"])))
+    g = cbct.Geometry(**kw, **extra)
+    assert g.symmetry()[0] != 4 and g.symmetry()[1]
+    rng = np.random.default_rng(500 + C)
+    vol = rng.random((C,) + g.vol_shape, dtype=np.float32)
+    y = rng.random((C,) + g.sino_shape, dtype=np.float32) * 20.0
+    ref = oracle_mod.fp(oracle_mod.Geom(**kw, **extra), vol.astype(np.float64))
+    out = torch.full((C,) + g.sino_shape, float("nan"), device="cuda")
+    g.fp(dev(vol), out, C)
+    got = out.cpu().numpy().astype(np.float64)
+    assert rel_l2(got, ref) <= 1e-5, rel_l2(got, ref)
+    assert max_rel(got, ref) <= 1e-4, max_rel(got, ref)
+    g.fp_residual(dev(vol), dev(y), out, C)
+    got = out.cpu().numpy().astype(np.float64)
+    assert np.max(np.abs(got - (ref - y))) <= 2e-5 * float(np.max(np.abs(ref)))
+
+
 @pytest.mark.parametrize("nz,C", [(21, 1), (40, 5), (7, 2)])
 def test_streamed_backprojectors_mirror_pairs(cbct, oracle_mod, nz, C):
     """A5 + z-mirror: with a work-set cap and a HOST volume the adjoint and the FDK backprojector fill each slab of the lower half together
