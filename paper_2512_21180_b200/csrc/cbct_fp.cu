@@ -389,6 +389,9 @@ __device__ __forceinline__ void fpm_sample(const float4 *__restrict__ packed, co
     M += fmaf(w00, lerpf(c00.z, c00.w, fx), fmaf(w10, lerpf(c10.z, c10.w, fx), fmaf(w01, lerpf(c01.z, c01.w, fx), w11 * lerpf(c11.z, c11.w, fx))));
 }
 
+// Measured at 256^3 / 400 views, 1 channel, jittered angles: 23.7 -> 18.9 ms; data stage 89 % busy at 5.5 cycles per
+// load (quad-packed: 6.4), L1 hit rate 97.4 %, 1.66e10 warp instructions (2.12e10).  The two-lanes-per-ray split of
+// fp4_pair_kernel measured slower here (19.7 ms: this kernel is closer to the issue limit, 76 % of the slots).
 // G: geometry of the lower slab (planes [0, G.z1)); nvh = rows with v <= 0 = ceil(nv / 2); CTA as fp_kernel
 template <int TU>
 __global__ void __launch_bounds__(32 * (FP_CTA_U / TU) * FPK_VPC)
