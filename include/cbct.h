@@ -133,7 +133,8 @@ int cbct_geom_destroy(cbct_geom *g);
  * vol: channels*nz*ny*nx floats (read), sino: channels*n_views*nv*nu floats (written).
  * Channels are independent.  Batching pays: groups of 4 channels share one re-laid-out copy of the volume and all
  * tap weights (and the backprojectors share their weights over up to 4 channels); a channel outside such a group
- * is projected through its four quarter-turn images when the geometry has that symmetry.  So a channel's bits may
+ * is projected through its four quarter-turn images when the geometry has that symmetry, else together with its
+ * z-mirror image when volume and detector rows are centred in z.  So a channel's bits may
  * differ between a batched and a single-channel call by fp32 rounding (1e-6 .. 1e-5 of the result's scale, the
  * error either call has against an exact evaluation), never by more. */
 int cbct_fp(const cbct_geom *g, const float *vol, float *sino, int32_t channels, void *cuda_stream);
