@@ -444,11 +444,11 @@ def main():
     names = {"fp": ("fp4_pair_kernel" if (C % 4 == 0 or quarter_turns)
                     else (tail_kernel if C < 4 else "fp4_pair_kernel+" + tail_kernel)),
              "adjoint": None, "fdk": "fdk_kernel"}
-    # adjoint (cbct_adjoint.cu: launch_gather_channels), on grids of 2 million base voxels or more: with rotation
+    # adjoint (cbct_adjoint.cu: launch_gather_channels), on grids of 200 000 base voxels or more: with rotation
     # symmetry, blocks of 4 (or 8) channels take the voxel kernel and the remaining 1-3 channels the column-walk kernel;
     # without it (irregular angle lists) the column-walk kernel takes every block
     images = rotations * (2 if mirror else 1)
-    large = g.n_vol // images >= 2000000
+    large = g.n_vol // images >= 200000
     tail = C % 4 if images == 8 else (C % 8) % 4
     if large and images <= 2:
         names["adjoint"] = "adjoint_column_kernel"

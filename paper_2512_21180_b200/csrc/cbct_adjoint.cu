@@ -405,6 +405,8 @@ static int launch_gather(cbct_geom *g, AdjGeom &G, const float *sinoI, float *vo
     return CBCT_OK;
 }
 
+static bool adjoint_uses_column(const cbct_geom *g, bool partial_ok);
+
 template <int NR, int NM>
 static int launch_gather_channels(cbct_geom *g, AdjGeom &G, const float *sinoI, float *vol, int channels,
                                   size_t sstride, size_t vstride, int vol_z_origin, float *partial, int nsplit,
@@ -413,9 +415,13 @@ static int launch_gather_channels(cbct_geom *g, AdjGeom &G, const float *sinoI, 
     int c = 0;
     // the partial-output workspace is sized for the regime of the grid (cbct_adjoint_partial_floats): 8 channels of
     // the voxel kernel on small grids, 2 channels of the column kernel on large ones
-    const bool small = cbct_adjoint_small_grid(g) && nsplit > 1;
-    float *const partial_voxel = small ? partial : nullptr;
-    const int nsplit_voxel = small ? nsplit : 1;
+    // (`nsplit` != 1 only says that partial outputs may be used: the group counts are the regimes' own)
+    const bool partial_ok = partial != nullptr && nsplit > 1;
+    const int nsplit_voxel = partial_ok ? cbct_adjoint_view_splits(g) : 1;
+    float *const partial_voxel = nsplit_voxel > 1 ? partial : nullptr;
+    const int nsplit_column = partial_ok ? cbct_adjoint_column_splits(g) : 1;
+    float *const partial_column = nsplit_column > 1 ? partial : nullptr;
+    const bool small = !adjoint_uses_column(g, partial_ok);
     while (c < channels) {
         int left = channels - c, rc;
         const float *s = sinoI + c * sstride;
@@ -434,7 +440,7 @@ static int launch_gather_channels(cbct_geom *g, AdjGeom &G, const float *sinoI, 
             // instead of 4 scalar loads); groups cover channels [0, 4 ci_groups)
             int ci = 1;
             if (NR == 1 && cb >= 4 && sino_ci && c % 4 == 0 && c + cb <= 4 * ci_groups) { ci = 4; s = sino_ci + c * sstride; }
-            rc = cbct_launch_adjoint_column(g, G, NR, NM, cb, ci, s, v, sstride, vstride, vol_z_origin, partial, nsplit, st);
+            rc = cbct_launch_adjoint_column(g, G, NR, NM, cb, ci, s, v, sstride, vstride, vol_z_origin, partial_column, nsplit_column, st);
             if (rc == CBCT_OK) { c += cb; continue; }
             if (rc != 1) return rc;
         }
@@ -490,22 +496,40 @@ static size_t adjoint_base_threads(const cbct_geom *g)
     return threads ? threads : 1;
 }
 
+// Two regimes of view groups.  VOXEL kernel: grids of fewer than 2 million base voxels do not fill the GPU with one
+// thread per base voxel, so the views of a launch are split over up to 32 groups of CTAs.  COLUMN kernel: grids of
+// ADJ_COLUMN_GRID base voxels or more give it enough CTAs (tiles x chunks x 8 view groups; measured at 128^3 / 400
+// views: 10.0 against 11.7 ms at full symmetry, 33 against 40 ms (1 channel) and 33 against 56 ms (4 channels) with
+// jittered angles; at 64^3 the voxel kernel wins, 7.5 against 28 ms); its 8 groups are there to even out the load.
+#ifndef ADJ_COLUMN_GRID
+#define ADJ_COLUMN_GRID 200000
+#endif
 bool cbct_adjoint_small_grid(const cbct_geom *g) { return adjoint_base_threads(g) < 2000000; }
+static bool column_grid(const cbct_geom *g) { return adjoint_base_threads(g) >= ADJ_COLUMN_GRID; }
 
-int cbct_adjoint_view_splits(const cbct_geom *g)
+int cbct_adjoint_view_splits(const cbct_geom *g)   // voxel kernel
 {
     const cbct_geom_desc &d = g->d;
-    if (d.n_views > CBCT_VIEWS_PER_LAUNCH && cbct_adjoint_small_grid(g)) return 1;
-    if (!cbct_adjoint_small_grid(g)) {
-        // large grids (column kernel): 8 view groups per tile even out the load of the SMs; not under a work-set
-        // cap (the partial outputs are whole volumes) and not for a handful of views
-        if (d.max_workset_bytes != 0 || d.n_views < 64) return 1;
-        return d.n_views >= 128 ? 8 : 4;   // measured at 256^3 / 400 views, 1 channel: 21.1 (none), 18.6, 16.7, 16.0 ms
-    }
+    if (d.n_views > CBCT_VIEWS_PER_LAUNCH || !cbct_adjoint_small_grid(g)) return 1;
     size_t s = (2000000 + adjoint_base_threads(g) - 1) / adjoint_base_threads(g);
     if (s > 32) s = 32;
     if (s > (size_t)d.n_views / 8) s = (size_t)d.n_views / 8;
     return s < 1 ? 1 : (int)s;
+}
+
+int cbct_adjoint_column_splits(const cbct_geom *g)   // column kernel
+{
+    const cbct_geom_desc &d = g->d;
+    // not under a work-set cap (the partial outputs are whole volumes) and not for a handful of views
+    if (!column_grid(g) || d.max_workset_bytes != 0 || d.n_views < 64) return 1;
+    return d.n_views >= 128 ? 8 : 4;   // measured at 256^3 / 400 views, 1 channel: 21.1 (none), 18.6, 16.7, 16.0 ms
+}
+
+// Does a launch that may use partial outputs (`partial_ok`: device volume, whole plane range) route its small channel
+// blocks (and, without rotation symmetry, all blocks) to the column kernel?  Otherwise the voxel kernel's view groups.
+static bool adjoint_uses_column(const cbct_geom *g, bool partial_ok)
+{
+    return column_grid(g) || !(partial_ok && cbct_adjoint_view_splits(g) > 1);
 }
 
 // The column kernel's preconditions (cbct_adjoint_column.cu) from the geometry alone: the 6-sample window and the
@@ -523,7 +547,7 @@ static bool column_kernel_serves(const cbct_geom *g)
 int cbct_adjoint_channel_groups(const cbct_geom *g, int channels, bool device_volume)
 {
     if (g->sym_rot != 1 || channels < 4 || !column_kernel_serves(g)) return 0;
-    if (cbct_adjoint_small_grid(g) && device_volume && cbct_adjoint_view_splits(g) > 1) return 0;  // voxel kernel's view groups
+    if (!adjoint_uses_column(g, device_volume)) return 0;  // voxel kernel's view groups
     return channels / 4;
 }
 
@@ -541,13 +565,15 @@ int cbct_launch_interleave_channels(cbct_geom *g, const float *sino, float *out,
     return cbct_check_launch(g, "interleave_views_kernel");
 }
 
-// floats of workspace the partial outputs of `cbct_adjoint_view_splits(g)` view groups need
+// floats of workspace the partial outputs of the view groups need (both regimes; 0 = none)
 size_t cbct_adjoint_partial_floats(const cbct_geom *g)
 {
-    const int nsplit = cbct_adjoint_view_splits(g);
-    if (nsplit <= 1) return 0;
     const size_t nvol = (size_t)g->d.vol_nx * g->d.vol_ny * g->d.vol_nz;
-    return (cbct_adjoint_small_grid(g) ? (size_t)nsplit * 8 : (size_t)16) * nvol;   // large grids: nsplit * CB <= 16
+    const int nv = cbct_adjoint_view_splits(g), nc = cbct_adjoint_column_splits(g);
+    size_t vols = 0;
+    if (nv > 1) vols = (size_t)nv * 8;           // voxel kernel: up to 8 channels per launch
+    if (nc > 1 && vols < 16) vols = 16;          // column kernel: nsplit * CB <= 16
+    return vols * nvol;
 }
 
 // `partial` (nsplit > 1 only): workspace of nsplit * 8 * nx * ny * nz floats; used when the launch covers the

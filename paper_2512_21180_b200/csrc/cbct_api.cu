@@ -415,10 +415,11 @@ static int adjoint_impl(const cbct_geom *gc, const float *sino, float *vol, int3
         }
     }
     // the views of a launch split over groups of CTAs (partial outputs in workspace, then reduced)
-    int nsplit = cx.kv == MEM_DEVICE ? cbct_adjoint_view_splits(g) : 1;
+    const size_t partial_floats = cx.kv == MEM_DEVICE ? cbct_adjoint_partial_floats(g) : 0;
+    const int nsplit = partial_floats ? 2 : 1;   // "partial outputs may be used": the launcher picks the group counts
     float *partial = nullptr;
-    if (nsplit > 1) {
-        rc = ensure(&g->ws_vol, &g->ws_vol_bytes, cbct_adjoint_partial_floats(g) * sizeof(float));
+    if (partial_floats) {
+        rc = ensure(&g->ws_vol, &g->ws_vol_bytes, partial_floats * sizeof(float));
         if (rc) return rc;
         partial = g->ws_vol;
     }

@@ -130,7 +130,8 @@ int cbct_launch_adjoint(cbct_geom *g, const float *sino_src, float *vol, int cha
 int cbct_adjoint_channel_groups(const cbct_geom *g, int channels, bool device_volume);
 int cbct_launch_interleave_channels(cbct_geom *g, const float *sino, float *out, int groups, const float *weights,
                                     cudaStream_t st);
-int cbct_adjoint_view_splits(const cbct_geom *g);   // view groups per tile of the adjoint (1 = none)
+int cbct_adjoint_view_splits(const cbct_geom *g);   // view groups of the adjoint's voxel kernel on small grids (1 = none)
+int cbct_adjoint_column_splits(const cbct_geom *g); // view groups per tile of the adjoint's column kernel (1 = none)
 bool cbct_adjoint_small_grid(const cbct_geom *g);    // fewer than 2 million base voxels: the voxel kernel splits views
 size_t cbct_adjoint_partial_floats(const cbct_geom *g);  // workspace floats of the view groups' partial outputs
 int cbct_launch_pad_sino(cbct_geom *g, const float *src, float *dst, int channels, cudaStream_t st);

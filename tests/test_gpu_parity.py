@@ -249,11 +249,14 @@ _HALFFAN_128 = dict(det_nu=128, det_nv=128, det_du_mm=3.2, det_dv_mm=3.2, det_of
     (dict(_HALFFAN_128, vol_nx=160, vol_ny=160, vol_nz=160, vox_mm=3.0, n_views=64, irregular=True), 5),  # NR 1, NM 2: blocks of 4 + 1
     (dict(_HALFFAN_128, vol_nx=128, vol_ny=128, vol_nz=128, vox_mm=4.0, n_views=64, vol_cz_mm=6.0, irregular=True), 9),  # none: 8 + 1
     (dict(_HALFFAN_128, vol_nx=128, vol_ny=128, vol_nz=128, vox_mm=4.0, n_views=64, det_off_v_mm=4.0, irregular=True), 6),  # none: 4 + 2
+    (dict(_HALFFAN_128, vol_nx=128, vol_ny=128, vol_nz=128, vox_mm=4.0, n_views=64), 1),   # 262 144 base voxels: column kernel
+    (dict(_HALFFAN_128, vol_nx=128, vol_ny=128, vol_nz=128, vox_mm=4.0, n_views=64), 5),   # ... 4 (voxel kernel, its own view groups) + 1
+    (dict(_HALFFAN_128, vol_nx=96, vol_ny=96, vol_nz=96, vox_mm=5.0, n_views=70, irregular=True), 6),   # 442 368: groups of 4 + 2
     (dict(det_nu=48, det_nv=48, det_du_mm=8.0, det_dv_mm=8.0, det_off_u_mm=100.0, vol_nx=256, vol_ny=256, vol_nz=256,
           vox_mm=2.0, n_views=1040), 1),   # more views than one launch chunk: the groups accumulate over the chunks
 ])
 def test_adjoint_column_kernel_with_view_groups(cbct, oracle_mod, over, C):
-    """Calls of fewer than 4 channels on grids of 2 million base voxels or more take the column-walk kernel
+    """Calls of fewer than 4 channels (and all calls without rotation symmetry) on grids of 200 000 base voxels or more take the column-walk kernel
     (cbct_adjoint_column.cu), and with 64 views or more its CTAs split the views into groups whose partial outputs
     are reduced afterwards.  Whole array against the oracle, every symmetry class, channel blocks of 2 and 1."""
     kw, extra = _symmetry_case(over)
