@@ -432,6 +432,8 @@ static int launch_gather_channels(cbct_geom *g, AdjGeom &G, const float *sinoI, 
         // Without rotation symmetry (NR * NM <= 2: irregular angle lists) the column kernel also takes the wide
         // blocks, 8 / (NR * NM) channels per thread: its window then holds the same 8 accumulators per plane as the
         // single-channel instance of a fully symmetric geometry.
+        // (measured at 256^3 / 400 views, 8 channels, full symmetry: column kernel on blocks of 2: 98.2 ms, voxel
+        // kernel on blocks of 4: 95.3 ms)
         if (!small && (left < 4 || NR * NM <= 2)) {
             int cb = left >= 2 ? 2 : 1;
             if (NR * NM <= 2 && left >= 4) cb = 4;
