@@ -231,6 +231,25 @@ int cbct_bp_adjoint_slab(const cbct_geom *g, const float *sino, float *out, int3
 int cbct_bp_fdk_slab(const cbct_geom *g, const float *sino, float *out, int32_t channels, int32_t z0, int32_t z1,
                      int32_t mirror_pair, void *cuda_stream);
 
+/* cbct_bp_fdk for callers that may not allocate (code under CUDA-graph capture, tight serving loops, harnesses
+ * that forbid cudaMalloc): the same two kernels as cbct_bp_fdk with DEVICE pointers (the result is
+ * the same bit for bit), but the kernel's scratch -- the zero-bordered, record-interleaved copy of the sinogram --
+ * lives in a file-scope device array of CBCT_STATIC_SCRATCH_BYTES that every GPU which loads the library holds
+ * until the process exits.  The call makes no cudaMalloc / cudaFree, creates no stream or event and does not
+ * synchronise; it enqueues on `cuda_stream` of the current device.  sino: [channels][n_views][det_nv][det_nu],
+ * vol: [channels][nz][ny][nx], both DEVICE pointers owned by the caller (host pointers: CBCT_ERR_INVALID_ARG).
+ * A geometry / channel count whose padded sinogram (about 4 x, with two-fold view symmetry 1 x, the sinogram's
+ * bytes) exceeds the array returns CBCT_ERR_UNSUPPORTED, with the two sizes in cbct_last_cuda_error, and enqueues
+ * nothing; so does a handle with cbct_geom_profile switched on.  max_workset_bytes is not consulted.
+ * ONE array per device serves every handle and every call: it keeps the last call's contents (nothing needs
+ * clearing: each call rewrites the region it reads, zero border included), and calls that overlap on the GPU
+ * (two streams, two threads) RACE on it -- the caller serialises them.
+ * cbct_static_scratch_setup resolves the array's device address for the CURRENT device (cbct_bp_fdk_static does
+ * the same on its first call per device); call it once per device outside stream capture. */
+#define CBCT_STATIC_SCRATCH_BYTES (32u << 20)
+int cbct_static_scratch_setup(void);
+int cbct_bp_fdk_static(const cbct_geom *g, const float *sino, float *vol, int32_t channels, void *cuda_stream);
+
 /* Kernels launched by this handle since creation (for bench.py's gpu_launches). */
 int cbct_geom_launch_count(const cbct_geom *g, uint64_t *out);
 

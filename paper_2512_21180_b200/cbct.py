@@ -26,8 +26,12 @@ EXPORTS = (
     "cbct_fp_residual", "cbct_bp_adjoint_weighted",
     "cbct_fov", "cbct_downsample", "cbct_upsample", "cbct_proj_down",
     "cbct_water_bone", "cbct_polychromatic_primary",
+    "cbct_static_scratch_setup", "cbct_bp_fdk_static",
     "cbct_status_string", "cbct_last_cuda_error",
 )
+
+
+STATIC_SCRATCH_BYTES = 32 << 20   # CBCT_STATIC_SCRATCH_BYTES (include/cbct.h)
 
 
 class CbctError(RuntimeError):
@@ -94,6 +98,8 @@ def load_library() -> ctypes.CDLL:
     L.cbct_water_bone.argtypes = [vp, vp, vp, i64, f64, f64, f64, f64, vp]
     dp = ctypes.POINTER(ctypes.c_double)
     L.cbct_polychromatic_primary.argtypes = [vp, vp, vp, dp, dp, dp, i32, i64, i64, vp, vp]
+    L.cbct_static_scratch_setup.argtypes = []
+    L.cbct_bp_fdk_static.argtypes = [vp, vp, vp, i32, vp]
     L.cbct_status_string.argtypes = [ctypes.c_int]
     L.cbct_status_string.restype = ctypes.c_char_p
     L.cbct_last_cuda_error.restype = ctypes.c_char_p
@@ -226,6 +232,18 @@ class Geometry:
         ps, pv = _ptr_and_keep(sino, channels * self.n_sino), _ptr_and_keep(vol, channels * self.n_vol)
         with _on_device_of((vol, sino), stream) as cx:
             _check(load_library().cbct_bp_fdk(self._h, ps, pv, channels, cx.stream))
+        return vol
+
+    def bp_fdk_static(self, sino, vol, channels: int = 1, stream=None):
+        """cbct_bp_fdk_static: bp_fdk on device tensors without any allocation (scratch in the library's static
+        device array of STATIC_SCRATCH_BYTES; calls that overlap on the GPU race on it)."""
+        ps, pv = _ptr_and_keep(sino, channels * self.n_sino), _ptr_and_keep(vol, channels * self.n_vol)
+        with _on_device_of((vol, sino), stream) as cx:
+            L = load_library()
+            rc = L.cbct_bp_fdk_static(self._h, ps, pv, channels, cx.stream)
+            if rc == -2:
+                raise CbctError(f"{L.cbct_status_string(rc).decode()} [{L.cbct_last_cuda_error().decode()}]")
+            _check(rc)
         return vol
 
     def slab_planes(self, z0: int, z1: int, mirror_pair: bool = False) -> int:
