@@ -34,9 +34,12 @@
  *   - Every data pointer may be a DEVICE pointer or a HOST pointer (pinned or
  *     pageable); the library detects which with cudaPointerGetAttributes.
  *     Host buffers are staged through library-owned device workspace inside
- *     the call: without a work-set cap, as a pipeline over blocks of 2 channels
- *     (H2D copy / kernels / D2H copy on three streams, joined back into
- *     `cuda_stream` before the call's work ends); with a cap, by z-slabs (A5).
+ *     the call: without a work-set cap, as a pipeline over blocks of 1 to 4
+ *     channels (H2D copy / kernels / D2H copy on three streams, joined back
+ *     into `cuda_stream` before the call's work ends; the block widths follow
+ *     the kernels' channel grouping, so single channels may round differently
+ *     -- by fp32 summation order -- from the same call on device buffers);
+ *     with a cap, by z-slabs (A5).
  *     A call with any pageable host buffer synchronises the stream before
  *     returning.
  *   - Outputs are OVERWRITTEN, never accumulated into.

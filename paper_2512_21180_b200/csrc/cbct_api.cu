@@ -111,9 +111,13 @@ static int begin_call(const cbct_geom *gc, const void *vol, const void *sino, in
 // PCIe copies in both directions hide behind the kernels.  `inner(din, dout, c0, nc)` enqueues the
 // device implementation for channels [c0, c0 + nc) on the caller's stream.
 // ---------------------------------------------------------------------------
-template <class Inner>
+// `sched(c0, left)` = channels of the block that starts at channel c0 (clamped to [1, min(BK, left)]): the first
+// block's H2D copy and the last block's D2H copy are the only transfers no kernel hides, so a call whose kernels run
+// as fast on narrower blocks starts and ends with those (measured on config 4 through pinned buffers, 8 channels:
+// cbct_fp 135.5 -> see DESIGN.md s.6.4).
+template <class Inner, class Sched>
 static int blocked_call(CallCtx &cx, const float *in, size_t n_in, MemKind kin, float *out, size_t n_out, MemKind kout,
-                        Inner inner, int BK = 2)
+                        Inner inner, int BK, Sched sched)
 {
     cbct_geom *g = cx.g;
     cudaStream_t st = cx.st;
@@ -136,9 +140,13 @@ static int blocked_call(CallCtx &cx, const float *in, size_t n_in, MemKind kin, 
     CBCT_CUDA_TRY(cudaEventRecord(ev0, st));
     CBCT_CUDA_TRY(cudaStreamWaitEvent(g->h2d_stream, ev0, 0));
     CBCT_CUDA_TRY(cudaStreamWaitEvent(g->d2h_stream, ev0, 0));
-    const int nb = (channels + BK - 1) / BK;
-    for (int b = 0; b < nb; ++b) {
-        const int i = b & 1, c0 = b * BK, nc = channels - c0 < BK ? channels - c0 : BK;
+    int nb = 0;
+    for (int b = 0, c0 = 0, nc = 0; c0 < channels; ++b, c0 += nc, nb = b) {
+        const int i = b & 1, left = channels - c0;
+        nc = sched(c0, left);
+        if (nc > BK) nc = BK;
+        if (nc > left) nc = left;
+        if (nc < 1) nc = 1;
         const float *din = in + (size_t)c0 * n_in;
         float *dout = out + (size_t)c0 * n_out;
         if (kin != MEM_DEVICE) {
@@ -192,7 +200,9 @@ static int fp_impl(const cbct_geom *gc, const float *vol, const float *y, float 
                             [&](const float *dv, float *ds, int c0, int nc) {
                                 return fp_impl(gc, dv, y ? y + (size_t)c0 * cx.nsino : nullptr, ds, nc, stream);
                             },
-                            channels >= 4 ? 4 : 2);  // blocks of 4 channels take the channel-interleaved kernel
+                            channels >= 4 ? 4 : 2,  // blocks of 4 channels take the channel-interleaved kernel ...
+                            // ... unless single channels run as fast (through their quarter-turn images)
+                            [&](int, int) { return cbct_fp_single_channel_is_fast(g) ? 1 : 4; });
 
     float *d_sino = sino;
     if (cx.ks != MEM_DEVICE) {
@@ -375,7 +385,13 @@ static int adjoint_impl(const cbct_geom *gc, const float *sino, float *vol, int3
                             [&](const float *ds, float *dv, int, int nc) {
                                 return adjoint_impl(gc, ds, dv, nc, stream, weighted);
                             },
-                            channels >= 4 ? 4 : 2);  // blocks of 4 channels take the 32-accumulator kernel
+                            channels >= 4 ? 4 : 2,  // blocks of 4 channels take the 32-accumulator kernel
+                            // at full symmetry on large grids blocks of 2 (column-walk kernel) cost 3 % more per
+                            // channel: the call starts and ends with one
+                            [&](int c0, int left) {
+                                if (!cbct_adjoint_pairs_are_fast(g)) return 4;
+                                return c0 > 0 && left >= 6 ? 4 : 2;
+                            });
 
     const float *d_sino = sino;
     if (cx.ks != MEM_DEVICE) {
@@ -455,7 +471,8 @@ extern "C" int cbct_bp_fdk(const cbct_geom *gc, const float *sino, float *vol, i
     cudaStream_t st = cx.st;
     if ((cx.kv != MEM_DEVICE || cx.ks != MEM_DEVICE) && g->d.max_workset_bytes == 0)
         return blocked_call(cx, sino, cx.nsino, cx.ks, vol, cx.nvol, cx.kv,
-                            [&](const float *ds, float *dv, int, int nc) { return cbct_bp_fdk(gc, ds, dv, nc, stream); });
+                            [&](const float *ds, float *dv, int, int nc) { return cbct_bp_fdk(gc, ds, dv, nc, stream); },
+                            2, [&](int, int) { return g->sym_rot == 1 ? 2 : 1; });  // the kernel takes 1 channel per launch (2 without rotation symmetry)
 
     // zero-bordered, rotation-interleaved copy of the sinogram (cbct_fdk.cu)
     const size_t psino = cbct_padded_sino_floats(g) * channels;

@@ -441,6 +441,8 @@ size_t cbct_packed_volume_cells(const RayGeom &r) { return (size_t)r.px * r.py *
 static size_t packed_tail_offset(const RayGeom &r, int channels) { return (size_t)(channels / 4) * cbct_packed4_cells(r); }
 // channels left over by the groups of 4: their quarter-turn images when the geometry has that symmetry
 static bool tail_by_rotation(const cbct_geom *g, const RayGeom &r) { return g->sym_rot == 4 && r.nx == r.ny; }
+// single channels run as fast as groups of 4 (used by the HOST-buffer pipeline, cbct_api.cu)
+bool cbct_fp_single_channel_is_fast(const cbct_geom *g) { return g->sym_rot == 4 && g->d.vol_nx == g->d.vol_ny; }
 // geometry of the lower slab that the mirror-paired layout holds (planes [0, fpm_ztop] of the whole grid)
 static RayGeom mirror_raygeom(const cbct_geom *g) { return cbct_make_raygeom(g, 0, fpm_ztop(g->d.vol_nz) + 1); }
 // ... used for the channels left over by the groups of 4 when the whole volume is resident (a z-slab of a streamed
