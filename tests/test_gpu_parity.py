@@ -528,6 +528,45 @@ def test_config4_multichannel_sampled(cbct, oracle_mod):
     assert rel_l2(got, ref) <= 1e-5
 
 
+@pytest.mark.parametrize("name", ["pyramid_256_jitter", "pyramid_256_v402"])
+def test_scanner_angle_lists_single_channel_sampled(cbct, oracle_mod, name):
+    """The single-channel bench workloads without the quarter-turn symmetry between views (a seeded +-0.2 degree
+    jitter on 400 angles: z-mirror only; 402 equispaced views: two-fold rotation + z-mirror), at full size and in
+    the launch configuration bench.py times: mirror-paired forward cells, column-walk adjoint with view groups, FDK
+    quad / pair records.  Sampled rays and voxels (random + seams) one by one against the oracle, and the fp32
+    adjoint identity."""
+    cfg = synth.CONFIGS[name]
+    kw = synth.geom_kwargs(cfg)
+    og = oracle_mod.Geom(**kw)
+    vol, sino = synth.make_volume(cfg), synth.make_sinogram(cfg)
+    Ax, Aty, F = run_fp(cbct, kw, vol), run_adj(cbct, kw, sino), run_fdk(cbct, kw, sino)
+    _sampled_checks(oracle_mod, og, vol[0], sino[0], Ax[0], Aty[0], F[0], (101, 102, 103),
+                    n_rays=1500, n_adj=128, n_fdk=1500, tag="_" + name)
+    lhs, rhs = float(np.sum(Ax * sino)), float(np.sum(vol.astype(np.float64) * Aty))
+    record("identity_" + name, rel=abs(lhs - rhs) / abs(lhs))
+    assert abs(lhs - rhs) / abs(lhs) <= 1e-5, (lhs, rhs)
+
+
+@pytest.mark.parametrize("name", ["multichannel_256_jitter", "multichannel_256_v402"])
+def test_scanner_angle_lists_multichannel_sampled(cbct, oracle_mod, name):
+    """The 8-channel bench workloads without the quarter-turn symmetry, as bench.py launches them (jittered angles:
+    column-walk adjoint on channel-interleaved groups of 4, two FDK channels per thread; 402 views: 8-channel voxel
+    kernel): channels 0 (phantom), 2 and 7 (signed noise) on sampled outputs, the adjoint identity on every channel."""
+    cfg = synth.CONFIGS[name]
+    kw = synth.geom_kwargs(cfg)
+    og = oracle_mod.Geom(**kw)
+    vol, sino = synth.make_volume(cfg), synth.make_sinogram(cfg)
+    Ax, Aty, F = run_fp(cbct, kw, vol), run_adj(cbct, kw, sino), run_fdk(cbct, kw, sino)
+    for c in (0, 2, 7):
+        _sampled_checks(oracle_mod, og, vol[c], sino[c], Ax[c], Aty[c], F[c], (111 + c, 121 + c, 131 + c),
+                        n_rays=600, n_adj=48, n_fdk=600, tag="_%s_c%d" % (name, c))
+    for c in range(cfg["channels"]):
+        lhs = float(np.sum(Ax[c] * sino[c]))
+        rhs = float(np.sum(vol[c].astype(np.float64) * Aty[c]))
+        record("identity_%s_c%d" % (name, c), rel=abs(lhs - rhs) / abs(lhs))
+        assert abs(lhs - rhs) / abs(lhs) <= 1e-5, (c, lhs, rhs)
+
+
 def test_config5_large_streamed_sampled(cbct, oracle_mod):
     """Config 5: 512^3 at 1 mm, 4 channels, 720 views, 512^2 offset detector, volume in pinned HOST memory
     under a 1 GiB work-set cap (forces the z-slab streaming path, A5).  Channel 0 (phantom) and channel 1
