@@ -817,6 +817,32 @@ def test_next3_fused_residual_and_weighted_adjoint(cbct, oracle_mod, over, cap):
     assert rel_l2(vol.cpu().numpy().astype(np.float64), want) <= 1e-4
 
 
+@pytest.mark.parametrize("over,C", [
+    (dict(_HALFFAN_128, vol_nx=96, vol_ny=96, vol_nz=96, vox_mm=5.0, n_views=70, irregular=True), 6),   # groups of 4 (w fused into the channel interleave) + 2 (weighted planar copy)
+    (dict(_HALFFAN_128, vol_nx=128, vol_ny=128, vol_nz=128, vox_mm=4.0, n_views=64, vol_cz_mm=6.0, irregular=True), 9),  # no symmetry: 8 + 1
+    (dict(_HALFFAN_128, vol_nx=128, vol_ny=128, vol_nz=128, vox_mm=4.0, n_views=64), 3),   # full symmetry: w fused into the view interleave, column kernel 2 + 1
+])
+def test_next3_weighted_adjoint_on_the_column_kernel_paths(cbct, oracle_mod, over, C):
+    """cbct_bp_adjoint_weighted = P^T (w y) on grids large enough for the column-walk kernel: without rotation
+    symmetry w(u) is applied inside the channel-interleaving pass (groups of 4) AND in a weighted planar copy (the
+    channels left over), with it inside the view-interleaving pass.  Whole array against the oracle's composition."""
+    kw, extra = _symmetry_case(over)
+    g = cbct.Geometry(**kw, **extra)
+    og = oracle_mod.Geom(**kw, **extra)
+    rng = np.random.default_rng(500 + C)
+    y = rng.random((C,) + g.sino_shape, dtype=np.float32)
+    y[C // 2] -= 0.5
+    vol = torch.full((C,) + g.vol_shape, float("nan"), device="cuda")
+    g.bp_adjoint_weighted(dev(y), vol, C)
+    torch.cuda.synchronize()
+    got = vol.cpu().numpy().astype(np.float64)
+    want = oracle_mod.bp_adjoint(og, y.astype(np.float64) * oracle_mod.redundancy_weight(og))
+    for c in range(C):
+        assert rel_l2(got[c], want[c]) <= 1e-4, (c, rel_l2(got[c], want[c]))
+    assert peak_err(got, want) <= 1e-5, peak_err(got, want)
+    record("weighted_adjoint_column", rel_l2=rel_l2(got, want), peak=peak_err(got, want), C=C)
+
+
 @pytest.mark.parametrize("step", [0.2, 0.37, 0.75, 1.0])
 def test_other_ray_steps(cbct, oracle_mod, step):
     """step_vox other than 1/2 (the gather adjoint's sample window holds 2 sqrt 2 / step lattice points)."""
