@@ -197,8 +197,15 @@ def test_capped_handle_does_not_thrash_its_workspace():
     assert sizes[1] == sizes[0] and sizes[2] == sizes[0], sizes
 
 
+_BINNED_PANEL = dict(det_nu=128, det_nv=128, det_du_mm=3.2, det_dv_mm=3.2, det_off_u_mm=115.0)   # PAPER.md:61, binned
+
+
 @pytest.mark.parametrize("over", [dict(n_views=12), dict(n_views=12, vol_nz=27), dict(n_views=7, det_off_v_mm=3.0),
-                                  dict(n_views=10, vol_nx=30, det_off_u_mm=20.0)])
+                                  dict(n_views=10, vol_nx=30, det_off_u_mm=20.0),
+                                  # grids on which the shard of a real call takes the column-walk adjoint kernel
+                                  dict(_BINNED_PANEL, vol_nx=128, vol_ny=128, vol_nz=128, vox_mm=4.0, n_views=64),
+                                  dict(_BINNED_PANEL, vol_nx=96, vol_ny=96, vol_nz=97, vox_mm=5.0, n_views=70,
+                                       angles_rad="seeded")])
 def test_plane_range_exports_tile_the_whole_volume_calls(oracle_mod, over):
     """cbct_bp_adjoint_slab / cbct_bp_fdk_slab (the shard of a plane-sharded multi-GPU backprojection): ranges that
     tile [0, nz), plain and as z-mirror pairs, reassemble the whole-volume result (FDK bit for bit; the adjoint to
@@ -208,6 +215,8 @@ def test_plane_range_exports_tile_the_whole_volume_calls(oracle_mod, over):
     from paper_2512_21180_b200 import cbct
     kw = dict(synth.geom_kwargs(synth.CONFIGS["tiny"]))
     kw.update(over)
+    if kw.get("angles_rad") == "seeded":
+        kw["angles_rad"] = list(np.sort(np.random.default_rng(8).uniform(0, 2 * np.pi, kw["n_views"])))
     g = cbct.Geometry(**kw)
     og = oracle_mod.Geom(**kw)
     C = 3
