@@ -70,6 +70,9 @@ interleave_views_kernel(const float *__restrict__ in, float *__restrict__ out, i
 // exactly -t (a_v = lambda_U (v - v*) and v* moves by sdd / U per plane), so the horizontal part of every tap
 // weight and all the per-pixel set-up are shared by the ZT voxels, as is the pixel load: the way to fill the
 // accumulator budget when the call has too few channels.
+#ifndef ADJ_BATCH_LOADS
+#define ADJ_BATCH_LOADS (CB >= 4)
+#endif
 template <int NR, int NM, int CB, bool FINE, int ADJ_BZ, int MINB, int ZT>
 __global__ void __launch_bounds__(ADJ_BX *ADJ_BY *ADJ_BZ, MINB)
 adjoint_gather_kernel(const float *__restrict__ sinoI, float *__restrict__ vol, const __grid_constant__ AdjGeom G,
@@ -164,16 +167,6 @@ adjoint_gather_kernel(const float *__restrict__ sinoI, float *__restrict__ vol, 
                 // a_v - t in place of a_v
                 const float zb = fmaf(fabsf(v), zcull, 1.0f);
                 if (ZT == 1 ? fabsf(av) >= zb : (av <= -zb || av >= (float)(ZT - 1) + zb)) continue;
-                // 4 channels (the 32-accumulator instance): channel 0's pixels are requested before the weight arithmetic,
-                // which covers their latency, and each further channel's while the one before is used (software
-                // pipeline; the compiler otherwise places every load right before its first use, where 36 % of the
-                // stall samples sat): 49.5 -> 47.7 ms per launch.  With 8 channels it gains nothing.
-                constexpr bool PIPE = CB == 4;
-                float yc0[PIPE ? NR : 1], yc1[PIPE ? NR : 1];
-                if (PIPE) {
-                    load_views<NR>(sq + i0, reinterpret_cast<float (&)[NR]>(yc0));
-                    if (NM == 2) load_views<NR>(sq + i1, reinterpret_cast<float (&)[NR]>(yc1));
-                }
                 const float L = L2 * invL;
                 const float invg = L * inv_stepf;  // samples per unit lambda
                 const float g = G.step * invL;     // lambda per sample
@@ -214,44 +207,47 @@ adjoint_gather_kernel(const float *__restrict__ sinoI, float *__restrict__ vol, 
 #pragma unroll
                 for (int t = 0; t < ZT; ++t) any = any || W[t] != 0.f;
                 if (!any) continue;
-                if constexpr (PIPE) {
+                // All pixel loads of the ray are issued together, once its weight is known to be non-zero (24 % of the
+                // enumerated rays have none), then the 32 FMAs.  Measured on the 32-accumulator instance at 256^3 / 400
+                // views, per 4-channel launch: loads placed by the compiler right before their first use 49.5 ms;
+                // channel 0's requested before the weight arithmetic and the others pipelined behind it 47.5 ms (ptxas
+                // sinks them below the test anyway and keeps the staging registers); this form 45.3 ms.  The 8-channel
+                // instances gain as much (402 views, 8 channels: 114.6 -> 101.9 ms); with 1 or 2 channels it changes nothing.
+                constexpr bool BATCH = ADJ_BATCH_LOADS;
+                if constexpr (BATCH) {
+                    float ya[CB][NR], yb[NM == 2 ? CB : 1][NR];
 #pragma unroll
                     for (int cc = 0; cc < CB; ++cc) {
-                        float yn0[NR], yn1[NR];
-                        if (cc + 1 < CB) {   // next channel's pixels in flight while this one's are used
-                            load_views<NR>(sq + (cc + 1) * sino_cstride + i0, yn0);
-                            if (NM == 2) load_views<NR>(sq + (cc + 1) * sino_cstride + i1, yn1);
-                        }
+                        load_views<NR>(sq + cc * sino_cstride + i0, ya[cc]);
+                        if (NM == 2) load_views<NR>(sq + cc * sino_cstride + i1, yb[NM == 2 ? cc : 0]);
+                    }
+#pragma unroll
+                    for (int cc = 0; cc < CB; ++cc)
 #pragma unroll
                         for (int t = 0; t < ZT; ++t)
 #pragma unroll
                             for (int r = 0; r < NR; ++r) {
-                                accv[cc * ZT + t][r] = fmaf(W[t], yc0[PIPE ? r : 0], accv[cc * ZT + t][r]);
-                                if (NM == 2) accv[(NM - 1) * CB * ZT + cc * ZT + t][r] = fmaf(W[t], yc1[PIPE ? r : 0], accv[(NM - 1) * CB * ZT + cc * ZT + t][r]);
+                                accv[cc * ZT + t][r] = fmaf(W[t], ya[cc][r], accv[cc * ZT + t][r]);
+                                if (NM == 2) accv[(NM - 1) * CB * ZT + cc * ZT + t][r] = fmaf(W[t], yb[NM == 2 ? cc : 0][r], accv[(NM - 1) * CB * ZT + cc * ZT + t][r]);
                             }
-                        if (cc + 1 < CB) {
-#pragma unroll
-                            for (int r = 0; r < NR; ++r) { yc0[PIPE ? r : 0] = yn0[r]; if (NM == 2) yc1[PIPE ? r : 0] = yn1[r]; }
-                        }
-                    }
                 } else {
 #pragma unroll
-                for (int cc = 0; cc < CB; ++cc) {
-                    float y[NR];
-                    load_views<NR>(sq + cc * sino_cstride + i0, y);
-#pragma unroll
-                    for (int t = 0; t < ZT; ++t)
-#pragma unroll
-                        for (int r = 0; r < NR; ++r) accv[cc * ZT + t][r] = fmaf(W[t], y[r], accv[cc * ZT + t][r]);
-                    if (NM == 2) {
-                        load_views<NR>(sq + cc * sino_cstride + i1, y);
+                    for (int cc = 0; cc < CB; ++cc) {
+                        float y[NR];
+                        load_views<NR>(sq + cc * sino_cstride + i0, y);
 #pragma unroll
                         for (int t = 0; t < ZT; ++t)
 #pragma unroll
-                            for (int r = 0; r < NR; ++r)
-                                accv[(NM - 1) * CB * ZT + cc * ZT + t][r] = fmaf(W[t], y[r], accv[(NM - 1) * CB * ZT + cc * ZT + t][r]);
+                            for (int r = 0; r < NR; ++r) accv[cc * ZT + t][r] = fmaf(W[t], y[r], accv[cc * ZT + t][r]);
+                        if (NM == 2) {
+                            load_views<NR>(sq + cc * sino_cstride + i1, y);
+#pragma unroll
+                            for (int t = 0; t < ZT; ++t)
+#pragma unroll
+                                for (int r = 0; r < NR; ++r)
+                                    accv[(NM - 1) * CB * ZT + cc * ZT + t][r] = fmaf(W[t], y[r], accv[(NM - 1) * CB * ZT + cc * ZT + t][r]);
+                        }
                     }
-                }
                 }
             }
         }
