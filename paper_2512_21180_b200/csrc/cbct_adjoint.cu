@@ -73,14 +73,30 @@ interleave_views_kernel(const float *__restrict__ in, float *__restrict__ out, i
 #ifndef ADJ_BATCH_LOADS
 #define ADJ_BATCH_LOADS (CB >= 4)
 #endif
+#ifndef ADJ_QW_4X2
+#define ADJ_QW_4X2 true
+#endif
+#ifndef ADJ_DEFER
+#define ADJ_DEFER (CB == 4)
+#endif
 template <int NR, int NM, int CB, bool FINE, int ADJ_BZ, int MINB, int ZT>
 __global__ void __launch_bounds__(ADJ_BX *ADJ_BY *ADJ_BZ, MINB)
 adjoint_gather_kernel(const float *__restrict__ sinoI, float *__restrict__ vol, const __grid_constant__ AdjGeom G,
                       const __grid_constant__ ViewChunk V, int q0, int accumulate, size_t sino_cstride,
                       size_t vol_cstride, int vol_z_origin)
 {
-    const int ix = blockIdx.x * ADJ_BX + threadIdx.x;
-    const int iy = blockIdx.y * ADJ_BY + threadIdx.y;
+    // Lanes of a warp (8 x 4 voxels of one plane): a quarter-warp -- the unit the L1 data stage serves per cycle for
+    // LDG.128 -- covers 4 (x) x 2 (y) voxels, not 8 x 1: its pixels then span at most 1.92 (3 |sin| + |cos|) < 7
+    // detector columns, so no two of them share a 16-byte position in different lines (profiles/r1_l1_microbench.md).
+    // Simulated data-stage wavefronts per LDG.128 on config 4: 6.1 -> 4.6 (measured before: 6.4).
+    int lx = threadIdx.x, ly = threadIdx.y;
+    if (ADJ_QW_4X2) {
+        const int l = threadIdx.x + ADJ_BX * (threadIdx.y & 3), qw = l >> 3, i = l & 7;
+        lx = (i & 3) + 4 * (qw & 1);
+        ly = (threadIdx.y & ~3) + (i >> 2) + 2 * (qw >> 1);
+    }
+    const int ix = blockIdx.x * ADJ_BX + lx;
+    const int iy = blockIdx.y * ADJ_BY + ly;
     const int nzb = (G.bz1 - G.bz0 + ADJ_BZ * ZT - 1) / (ADJ_BZ * ZT);
     const int split = blockIdx.z / nzb;
     // plane blocks are launched from the top of the range downwards: with the z-mirror the base planes are the
@@ -145,6 +161,21 @@ adjoint_gather_kernel(const float *__restrict__ sinoI, float *__restrict__ vol, 
 #pragma unroll
             for (int r = 0; r < NR; ++r) accv[i][r] = 0.f;
 
+        // DEFER (instances that batch their loads): the pixels of a ray are requested when its weight is known and
+        // consumed only after the NEXT ray's weight arithmetic, which covers their latency (before: 35 % of the stall
+        // samples on the first FMAs behind the loads)
+        constexpr bool DEFER = ADJ_BATCH_LOADS && ADJ_DEFER && ZT == 1;
+        float pya[DEFER ? CB : 1][NR], pyb[DEFER && NM == 2 ? CB : 1][NR], pW = 0.f;
+        bool pending = false;
+        auto consume = [&]() {
+#pragma unroll
+            for (int cc = 0; cc < CB; ++cc)
+#pragma unroll
+                for (int r = 0; r < NR; ++r) {
+                    accv[cc][r] = fmaf(pW, pya[DEFER ? cc : 0][r], accv[cc][r]);
+                    if (NM == 2) accv[(NM - 1) * CB + cc][r] = fmaf(pW, pyb[DEFER && NM == 2 ? cc : 0][r], accv[(NM - 1) * CB + cc][r]);
+                }
+        };
         for (int iu = iu_lo; iu <= iu_hi; ++iu) {
             const float u = fmaf((float)iu, duf, u0f);
             const float au = lu * (dfu0 + (float)(iu - iu_lo));
@@ -214,7 +245,16 @@ adjoint_gather_kernel(const float *__restrict__ sinoI, float *__restrict__ vol, 
                 // sinks them below the test anyway and keeps the staging registers); this form 45.3 ms.  The 8-channel
                 // instances gain as much (402 views, 8 channels: 114.6 -> 101.9 ms); with 1 or 2 channels it changes nothing.
                 constexpr bool BATCH = ADJ_BATCH_LOADS;
-                if constexpr (BATCH) {
+                if constexpr (DEFER) {
+                    if (pending) consume();
+#pragma unroll
+                    for (int cc = 0; cc < CB; ++cc) {
+                        load_views<NR>(sq + cc * sino_cstride + i0, pya[DEFER ? cc : 0]);
+                        if (NM == 2) load_views<NR>(sq + cc * sino_cstride + i1, pyb[DEFER && NM == 2 ? cc : 0]);
+                    }
+                    pW = W[0];
+                    pending = true;
+                } else if constexpr (BATCH) {
                     float ya[CB][NR], yb[NM == 2 ? CB : 1][NR];
 #pragma unroll
                     for (int cc = 0; cc < CB; ++cc) {
@@ -251,6 +291,7 @@ adjoint_gather_kernel(const float *__restrict__ sinoI, float *__restrict__ vol, 
                 }
             }
         }
+        if (DEFER && pending) consume();
 #pragma unroll
         for (int i = 0; i < NM * CB * ZT; ++i) {
             rotate_views<NR>(accv[i], a);
