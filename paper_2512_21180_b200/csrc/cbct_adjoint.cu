@@ -197,7 +197,11 @@ adjoint_gather_kernel(const float *__restrict__ sinoI, float *__restrict__ vol, 
                 // inside the square |mu| sdd <= sqrt 2, so |e_z - a_v| = |mu v| <= sqrt 2 |v| / sdd; plane t has
                 // a_v - t in place of a_v
                 const float zb = fmaf(fabsf(v), zcull, 1.0f);
-                if (ZT == 1 ? fabsf(av) >= zb : (av <= -zb || av >= (float)(ZT - 1) + zb)) continue;
+                const bool zout = ZT == 1 ? fabsf(av) >= zb : (av <= -zb || av >= (float)(ZT - 1) + zb);
+                // DEFER: no divergent branch between a ray's loads and their use one ray later (ptxas makes a warp
+                // wait for its outstanding loads at such a branch: 21 % of the stall samples sat on this one), so the
+                // rows outside the z-window go through the weight arithmetic and are dropped with the zero weights
+                if (!(ADJ_BATCH_LOADS && ADJ_DEFER && ZT == 1) && zout) continue;
                 const float L = L2 * invL;
                 const float invg = L * inv_stepf;  // samples per unit lambda
                 const float g = G.step * invL;     // lambda per sample
@@ -237,7 +241,7 @@ adjoint_gather_kernel(const float *__restrict__ sinoI, float *__restrict__ vol, 
                 bool any = false;
 #pragma unroll
                 for (int t = 0; t < ZT; ++t) any = any || W[t] != 0.f;
-                if (!any) continue;
+                if (!any || ((ADJ_BATCH_LOADS && ADJ_DEFER && ZT == 1) && zout)) continue;
                 // All pixel loads of the ray are issued together, once its weight is known to be non-zero (24 % of the
                 // enumerated rays have none), then the 32 FMAs.  Measured on the 32-accumulator instance at 256^3 / 400
                 // views, per 4-channel launch: loads placed by the compiler right before their first use 49.5 ms;
