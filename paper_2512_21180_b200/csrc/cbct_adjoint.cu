@@ -594,15 +594,6 @@ int cbct_adjoint_channel_groups(const cbct_geom *g, int channels, bool device_vo
     return channels / 4;
 }
 
-// Blocks of 2 channels cost about as much per channel as blocks of 4 (column-walk kernel: 24.5 ms per pair against
-// 47.5 ms per 4 at 256^3 / 400 views): full symmetry, a grid the voxel kernel would not split, a detector the column
-// kernel serves, no work-set cap (the view groups' partial outputs).  Used by the HOST-buffer pipeline (cbct_api.cu).
-bool cbct_adjoint_pairs_are_fast(const cbct_geom *g)
-{
-    return g->sym_rot == 4 && g->sym_mirror_z && !cbct_adjoint_small_grid(g) && column_kernel_serves(g) &&
-           g->d.max_workset_bytes == 0 && g->d.n_views <= CBCT_VIEWS_PER_LAUNCH;
-}
-
 // out[gq][view][pix][k] = in[4 gq + k][view][pix]: the rotation-interleaving kernel with "views per rotation block"
 // = all views and "channels" = groups (weights != nullptr: times w(u), the fused P*(w y))
 int cbct_launch_interleave_channels(cbct_geom *g, const float *sino, float *out, int groups, const float *weights,

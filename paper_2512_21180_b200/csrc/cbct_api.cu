@@ -386,12 +386,10 @@ static int adjoint_impl(const cbct_geom *gc, const float *sino, float *vol, int3
                                 return adjoint_impl(gc, ds, dv, nc, stream, weighted);
                             },
                             channels >= 4 ? 4 : 2,  // blocks of 4 channels take the 32-accumulator kernel
-                            // at full symmetry on large grids blocks of 2 (column-walk kernel) cost 3 % more per
-                            // channel: the call starts and ends with one
-                            [&](int c0, int left) {
-                                if (!cbct_adjoint_pairs_are_fast(g)) return 4;
-                                return c0 > 0 && left >= 6 ? 4 : 2;
-                            });
+                            // (pairs at both ends of the call -- the column-walk kernel, 12.3 ms per channel -- paid
+                            // while blocks of 4 ran at 11.9 ms per channel; at 10.1 they no longer do: 8 channels
+                            // through pinned buffers 95.6 ms as 2 + 4 + 2, 93.5 ms as 4 + 4)
+                            [&](int, int) { return 4; });
 
     const float *d_sino = sino;
     if (cx.ks != MEM_DEVICE) {

@@ -130,7 +130,6 @@ int cbct_launch_adjoint(cbct_geom *g, const float *sino_src, float *vol, int cha
 int cbct_adjoint_channel_groups(const cbct_geom *g, int channels, bool device_volume);
 // block widths of the HOST-buffer pipeline (cbct_api.cu): is a narrower block as fast per channel as a block of 4?
 bool cbct_fp_single_channel_is_fast(const cbct_geom *g);   // cbct_fp.cu
-bool cbct_adjoint_pairs_are_fast(const cbct_geom *g);      // cbct_adjoint.cu
 int cbct_launch_interleave_channels(cbct_geom *g, const float *sino, float *out, int groups, const float *weights,
                                     cudaStream_t st);
 int cbct_adjoint_view_splits(const cbct_geom *g);   // view groups of the adjoint's voxel kernel on small grids (1 = none)

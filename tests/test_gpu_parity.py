@@ -899,10 +899,10 @@ def test_host_buffers_channel_pipeline(cbct, oracle_mod, pinned):
 
 
 def test_host_pipeline_block_schedule_full_size(cbct):
-    """Config 4 through pinned HOST buffers: the forward pipeline runs 8 single-channel blocks, the adjoint blocks
-    of 2, 4, 2 channels (column-walk kernel at both ends), the FDK backprojection 8 single blocks.  Each channel must
-    agree with the device-buffer call (groups of 4; checked against the oracle at this size in
-    test_config4_multichannel_sampled) to the rounding of two different fp32 summation orders."""
+    """Config 4 through pinned HOST buffers: the forward pipeline runs 8 single-channel blocks, the adjoint 2 blocks
+    of 4 channels, the FDK backprojection 8 single blocks.  Each channel must agree with the device-buffer call
+    (checked against the oracle at this size in test_config4_multichannel_sampled): bit for bit where the same kernel
+    runs, else (the forward's single channels) to the rounding of two different fp32 summation orders."""
     cfg = synth.CONFIGS["multichannel_256"]
     g = cbct.Geometry(**synth.geom_kwargs(cfg))
     C = 8
