@@ -29,6 +29,14 @@ def test_exports_match_header(cbct):
         assert getattr(lib, name) is not None
 
 
+def test_static_scratch_limit_matches_header(cbct):
+    """The binding's STATIC_SCRATCH_BYTES is the header's CBCT_STATIC_SCRATCH_BYTES (cbct_bp_fdk_static)."""
+    hdr = open(os.path.join(ROOT, "include", "cbct.h")).read()
+    m = re.search(r"#define\s+CBCT_STATIC_SCRATCH_BYTES\s+\((\d+)u\s*<<\s*(\d+)\)", hdr)
+    assert m, "CBCT_STATIC_SCRATCH_BYTES not found in include/cbct.h"
+    assert int(m.group(1)) << int(m.group(2)) == cbct.STATIC_SCRATCH_BYTES
+
+
 def test_status_strings(cbct):
     lib = cbct.load_library()
     assert lib.cbct_status_string(0) == b"CBCT_OK"
